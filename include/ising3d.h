@@ -1,0 +1,188 @@
+/*
+ * ising3d.h -- C ABI of the B200-native zero-temperature coarsening sweep
+ * of the periodic simple-cubic d=3 Ising model (arXiv 2305.12161).
+ *
+ * Citations are PAPER.md:<line> = /root/reference/PAPER.md; "D<n>" are the
+ * readings listed in DESIGN.md section 3 for everything
+ * the paper leaves open.
+ *
+ * The method (what every call below computes)
+ * -------------------------------------------
+ *  - Lattice: s(x,y,z) in {-1,+1}, 0 <= x,y,z < L, periodic in all three
+ *    directions, nearest-neighbour coupling J = 1.
+ *  - Start: iid +-1 spins with p = 1/2, i.e. T = infinity, m ~ 0.
+ *  - Site rule, T -> 0 Glauber acceptance, eq. (6) PAPER.md:105-108:
+ *    Delta E = 2 s_i sum_nn s_j;  flip if Delta E < 0, keep if Delta E > 0,
+ *    flip with probability 1/2 if Delta E = 0 (here: iff the site's Philox bit
+ *    is 1, D2/D5).
+ *  - Sweep = checkerboard "01 cycle": all sites with
+ *    (x+y+z) even ("black", colour 0) concurrently, then all sites with
+ *    (x+y+z) odd ("white", colour 1), which see the updated black sites.
+ *    One sweep = N = L^3 proposals = 1 MCS.
+ *  - Measurements: N_up, the antiparallel-pair counts A_mu(r) along the three
+ *    axes for r = 0..L/2 (eq. (2) PAPER.md:43 reduced to integers, D8), the
+ *    number of broken nearest-neighbour bonds (interface energy
+ *    E = -3N + 2 n_broken), the axis-averaged C(r,t) and ell(t) from
+ *    C(ell,t) = c, c = 0.5 (D9).
+ *
+ * Canonical packed state (D3) -- the format of get_state / set_state
+ * -------------------------------------------------------------------
+ *  colour c = (x+y+z) mod 2.  Inside row (y,z) the colour-c sites are
+ *  x = 2k + o, o = (y+z+c) mod 2, k = x>>1 = 0..L/2-1.  Bit index inside
+ *  colour c: b = (z*L + y)*(L/2) + k; 32-bit word w = b>>5, bit j = b&31
+ *  (LSB = smallest k); bit value 1 <=> s = +1.  One replica = colour-0 words
+ *  (L^3/64 of them) followed by colour-1 words; replicas follow one another.
+ *  Words per replica: L^3/32.
+ *
+ * Random bits (D5)
+ * ----------------
+ *  Philox4x32-10, key = (seed & 0xFFFFFFFF, seed >> 32) (the replica's seed),
+ *  counter = (q, t, c, tag): q = b>>7 the 128-spin group inside the colour,
+ *  t = 0-based index of the sweep being executed, c = colour being updated,
+ *  tag = 0 for tie bits, 1 for the initial configuration (with t = 0).
+ *  Output word i (0..3) bit j belongs to the spin at bit index 128q + 32i + j.
+ *  Counter based: results never depend on thread order or launch shape.
+ *
+ * General conventions
+ * -------------------
+ *  - Every function returns ISING3D_OK (0) or a negative error code; no
+ *    exception or abort crosses this boundary.  ising3d_last_error() gives a
+ *    thread-local, never-NULL description of the last failure.
+ *  - "host" / "device" is stated for every pointer.  The library owns all
+ *    device memory it allocates and frees it in ising3d_free().
+ *  - Handles are not thread safe; distinct handles are independent.
+ *  - There is no CPU fallback: without a CUDA device every compute call
+ *    fails with ISING3D_ECUDA.
+ *  - L must be a multiple of 64 with 64 <= L <= 4096; 1 <= n_rep.
+ */
+#ifndef ISING3D_H_
+#define ISING3D_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ISING3D_OK      0
+#define ISING3D_EINVAL (-1)   /* bad argument (null pointer, bad L, n_rep, buffer too small,
+                                 sweep counter would pass 2^32-1)                        */
+#define ISING3D_ENOMEM (-2)   /* device or host allocation failed                         */
+#define ISING3D_ECUDA  (-3)   /* CUDA runtime error; text in ising3d_last_error()         */
+
+/* sweep-kernel variants (ising3d_set_variant) */
+#define ISING3D_VARIANT_AUTO    0   /* fused kernel where the shape allows, else generic */
+#define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
+#define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
+
+typedef struct ising3d ising3d_t;   /* opaque */
+
+/*
+ * Measurement record.  All arrays are HOST memory allocated by the CALLER;
+ * the caller sets L, n_rep (must match the handle), c_intercept and the
+ * pointers; ising3d_measure fills sweep and the arrays.
+ */
+typedef struct {
+    int32_t   L, n_rep;
+    uint64_t  sweep;        /* out: completed sweeps at the time of measurement           */
+    uint64_t *n_up;         /* [n_rep]              number of +1 spins (D8)               */
+    uint64_t *n_broken;     /* [n_rep]              antiparallel n.n. bonds = sum_mu A_mu(1) */
+    uint64_t *antipar;      /* [n_rep][3][L/2+1]    A_mu(r), mu = x,y,z; A_mu(0) = 0      */
+    double   *C;            /* [n_rep][L/2+1] or NULL   eq. (2), axis-averaged, fp64 (D9) */
+    double   *ell;          /* [n_rep] or NULL          first C = c crossing, NaN if none */
+    double    c_intercept;  /* 0.5 in the paper; other values: Table II     */
+} ising3d_meas_t;
+
+/* Device bytes needed by a handle with caller-provided memory
+ * (ising3d_init_batch_with_buffer).  0 if L / n_rep are invalid. */
+size_t ising3d_required_bytes(int L, int n_rep);
+
+/* Number of 32-bit words of the canonical packed state of ONE replica: L^3/32. */
+size_t ising3d_words_per_replica(int L);
+
+/*
+ * Create one lattice in the T = infinity start of `seed` (D6), sweep = 0.
+ * PAPER.md:45.  *h is written only on success.  Runs on the legacy default
+ * stream until ising3d_set_stream is called; the handle is created on the
+ * CUDA device current at the time of the call.
+ */
+int ising3d_init(ising3d_t **h, int L, uint64_t seed);
+
+/*
+ * n_rep independent lattices ("independent realizations"),
+ * replica i seeded with seeds[i] (HOST array of n_rep entries, copied).
+ * All replicas advance in the same launches.  Replica i is bit-identical to
+ * a single-lattice handle created with seeds[i].
+ */
+int ising3d_init_batch(ising3d_t **h, int L, int n_rep, const uint64_t *seeds);
+
+/*
+ * Same, in caller-provided DEVICE memory (e.g. a torch tensor): `dev_buf`
+ * must be 256-byte aligned and hold >= ising3d_required_bytes(L, n_rep);
+ * it stays owned by the caller and must outlive the handle.  `cuda_stream`
+ * is a cudaStream_t (may be NULL = legacy default stream); the initial state
+ * is generated on that stream.
+ */
+int ising3d_init_batch_with_buffer(ising3d_t **h, int L, int n_rep, const uint64_t *seeds,
+                                   void *dev_buf, size_t dev_bytes, void *cuda_stream);
+
+/* Re-generate the T = infinity start (same seeds) and reset sweep to 0. Async. */
+int ising3d_reset(ising3d_t *h);
+
+/* Use `cuda_stream` (a cudaStream_t owned by the caller) for all later work. */
+int ising3d_set_stream(ising3d_t *h, void *cuda_stream);
+
+/* Choose the sweep kernel (ISING3D_VARIANT_*).  EINVAL if the shape does not
+ * support the requested variant.  All variants give bit-identical states. */
+int ising3d_set_variant(ising3d_t *h, int variant);
+
+/*
+ * Run n_sweeps checkerboard sweeps (eq. (6)).
+ * Asynchronous on the handle's stream; no host synchronisation inside.
+ * The sweep counter advances by n_sweeps; EINVAL if it would pass 2^32-1.
+ */
+int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);
+
+/*
+ * Integer measurements + fp64 post-processing (D8, D9; eq. (2) PAPER.md:43,
+ * ell from C = c PAPER.md:51).  Synchronises the handle's stream.  Does not
+ * change the state or the sweep counter.
+ */
+int ising3d_measure(ising3d_t *h, ising3d_meas_t *out);
+
+/*
+ * Copy the canonical packed state (D3) to / from HOST memory.
+ * n_words must equal n_rep * L^3/32.  Both synchronise the stream.
+ * set_state also sets the sweep counter (the next sweep executed has index
+ * `sweep`), which with the counter-based RNG resumes a run exactly.
+ */
+int ising3d_get_state(ising3d_t *h, uint32_t *words, size_t n_words, uint64_t *sweep);
+int ising3d_set_state(ising3d_t *h, const uint32_t *words, size_t n_words, uint64_t sweep);
+
+/* Same with DEVICE pointers (device-to-device copies on the handle's stream,
+ * asynchronous).  Used to keep inputs resident in HBM.                        */
+int ising3d_get_state_device(ising3d_t *h, uint32_t *dev_words, size_t n_words, uint64_t *sweep);
+int ising3d_set_state_device(ising3d_t *h, const uint32_t *dev_words, size_t n_words, uint64_t sweep);
+
+/* Introspection: shape, completed sweeps, kernels launched so far by this handle. */
+int      ising3d_L(const ising3d_t *h);
+int      ising3d_n_rep(const ising3d_t *h);
+uint64_t ising3d_sweep_count(const ising3d_t *h);
+uint64_t ising3d_launch_count(const ising3d_t *h);
+/* name of the sweep kernel the handle currently dispatches to ("generic", "fused", ...) */
+const char *ising3d_variant_name(const ising3d_t *h);
+
+/* Block until all work queued on the handle's stream is done. */
+int ising3d_sync(ising3d_t *h);
+
+/* Release the handle and all memory the library allocated for it. NULL is a no-op. */
+void ising3d_free(ising3d_t *h);
+
+/* Thread-local description of the last error on this thread; never NULL. */
+const char *ising3d_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING3D_H_ */

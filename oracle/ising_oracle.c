@@ -1,0 +1,408 @@
+/*
+ * oracle/ising_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, site-by-site CPU statement of what the hot path of
+ * arXiv 2305.12161 computes: the zero-temperature single-spin-flip
+ * checkerboard sweep of the periodic simple-cubic d=3 Ising model and the
+ * integer measurements behind energy, magnetisation and C(r,t).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may build, load or call this file.  It shares no code,
+ * header, table or constant generator with paper_2305_12161_b200/csrc (the
+ * CUDA path); the two meet only in the tests, which compare their outputs.
+ *
+ * One int8 per spin, literal Delta-E rule, literal modular neighbour indexing.
+ * No blocking, no bit tricks, no fusion: every function is meant to be checked
+ * against the cited passage by eye.
+ *
+ * Citations are PAPER.md:<line> and SURVEY.md
+ * section 8(c) definitions D1..D9 (the readings taken where the paper is
+ * silent; they are listed again in DESIGN.md).
+ *
+ * Pins (tests/test_oracle_*.py, all run with -m "not gpu"):
+ *   orc_philox4x32_10   : known-answer vectors, NVIDIA's curand host path,
+ *                         big-integer Python restatement
+ *   orc_half_sweep      : exhaustive 2^6 x 2 x 2 site table, brute-force
+ *                         H(flipped)-H(config) variant on L=4,6,8, closed
+ *                         forms (Neel state, single spin, 2x2x2 cube), fixed
+ *                         points, order independence, energy monotonicity
+ *   orc_init_random     : bit statistics, independent Python restatement
+ *   orc_measure         : closed forms (slab, all-up), translation and axis
+ *                         permutation invariance, numpy restatement
+ *   orc_postprocess     : closed forms, hand-worked example
+ *   orc_export/import   : round trip, independent Python packer
+ * No function here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------ */
+/* D5: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).              */
+/* counter (c0,c1,c2,c3), key (k0,k1), all uint32.                     */
+/* One round: p0 = M0*c0, p1 = M1*c2 (64-bit products);                */
+/*   new counter = (hi(p1)^c1^k0, lo(p1), hi(p0)^c3^k1, lo(p0)).       */
+/* Ten rounds; the key is bumped by (W0,W1) between rounds (9 times).  */
+/* ------------------------------------------------------------------ */
+#define ORC_PHILOX_M0 0xD2511F53u
+#define ORC_PHILOX_M1 0xCD9E8D57u
+#define ORC_PHILOX_W0 0x9E3779B9u
+#define ORC_PHILOX_W1 0xBB67AE85u
+
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) {
+            k0 += ORC_PHILOX_W0;
+            k1 += ORC_PHILOX_W1;
+        }
+        uint64_t p0 = (uint64_t)ORC_PHILOX_M0 * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)ORC_PHILOX_M1 * (uint64_t)c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* ------------------------------------------------------------------ */
+/* The lattice: D1.  s[(z*L + y)*L + x] in {-1,+1}, periodic, L even.  */
+/* ------------------------------------------------------------------ */
+typedef struct {
+    int      L;
+    uint64_t seed;
+    uint32_t sweep;      /* completed sweeps (MCS) */
+    int8_t  *s;
+} orc_t;
+
+static inline size_t orc_idx(const orc_t *o, int x, int y, int z)
+{
+    return ((size_t)z * (size_t)o->L + (size_t)y) * (size_t)o->L + (size_t)x;
+}
+
+/* a mod L for -L <= a < 2L (all that periodic neighbours and r <= L/2 need) */
+static inline int orc_mod(int a, int L)
+{
+    if (a >= L) return a - L;
+    if (a < 0)  return a + L;
+    return a;
+}
+
+orc_t *orc_create(int L, uint64_t seed)
+{
+    if (L < 4 || (L & 1)) return NULL;
+    orc_t *o = (orc_t *)calloc(1, sizeof(orc_t));
+    if (!o) return NULL;
+    o->L = L;
+    o->seed = seed;
+    o->sweep = 0;
+    o->s = (int8_t *)malloc((size_t)L * L * L);
+    if (!o->s) { free(o); return NULL; }
+    memset(o->s, 1, (size_t)L * L * L);   /* all up until initialised */
+    return o;
+}
+
+void orc_free(orc_t *o)
+{
+    if (!o) return;
+    free(o->s);
+    free(o);
+}
+
+int8_t  *orc_spins(orc_t *o)            { return o->s; }
+uint32_t orc_get_sweep(const orc_t *o)  { return o->sweep; }
+void     orc_set_sweep(orc_t *o, uint32_t t) { o->sweep = t; }
+void     orc_set_seed(orc_t *o, uint64_t seed) { o->seed = seed; }
+
+/* ------------------------------------------------------------------ */
+/* D3: canonical packed position of a site.                            */
+/*   colour c = (x+y+z) mod 2; k = x>>1;                               */
+/*   bit index inside colour c: b = (z*L + y)*(L/2) + k;               */
+/*   group q = b>>7, word-in-group i = (b>>5)&3, bit j = b&31.         */
+/* ------------------------------------------------------------------ */
+static inline uint64_t orc_bit_index(int L, int x, int y, int z)
+{
+    return ((uint64_t)z * (uint64_t)L + (uint64_t)y) * (uint64_t)(L / 2) + (uint64_t)(x >> 1);
+}
+
+/* D5 keying: key = (seed lo, seed hi); counter = (q, t, c, tag);
+ * tag 0 = tie bits of sweep t, tag 1 = initial configuration (t = 0).
+ * The site's bit is bit j of output word i.                            */
+int orc_site_bit(uint64_t seed, int L, int x, int y, int z, uint32_t t, uint32_t tag)
+{
+    uint32_t c = (uint32_t)((x + y + z) & 1);
+    uint64_t b = orc_bit_index(L, x, y, z);
+    uint32_t ctr[4] = { (uint32_t)(b >> 7), t, c, tag };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    orc_philox4x32_10(ctr, key, out);
+    return (int)((out[(b >> 5) & 3] >> (b & 31)) & 1u);
+}
+
+/* D6 ("random spin configurations (with magnetization m ~ 0)"):
+ * spin = +1 iff its Philox(tag=1, t=0) bit is 1.                       */
+void orc_init_random(orc_t *o)
+{
+    const int L = o->L;
+    #pragma omp parallel for schedule(static)
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x)
+                o->s[orc_idx(o, x, y, z)] =
+                    orc_site_bit(o->seed, L, x, y, z, 0u, 1u) ? (int8_t)1 : (int8_t)-1;
+    o->sweep = 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* D2: the T -> 0 Glauber rule, eq. (6):              */
+/*   Delta E < 0 : accept;  Delta E > 0 : reject;                      */
+/*   Delta E = 0 : accept with probability 1/2 (here: iff the site's   */
+/*   random bit is 1).  H = -sum_<ij> s_i s_j, so flipping s_i changes */
+/*   the energy by Delta E = 2 s_i sum_{j in nn(i)} s_j. */
+/* ------------------------------------------------------------------ */
+static inline void orc_update_site(orc_t *o, int x, int y, int z, uint32_t t)
+{
+    const int L = o->L;
+    int h = o->s[orc_idx(o, orc_mod(x + 1, L), y, z)]
+          + o->s[orc_idx(o, orc_mod(x - 1, L), y, z)]
+          + o->s[orc_idx(o, x, orc_mod(y + 1, L), z)]
+          + o->s[orc_idx(o, x, orc_mod(y - 1, L), z)]
+          + o->s[orc_idx(o, x, y, orc_mod(z + 1, L))]
+          + o->s[orc_idx(o, x, y, orc_mod(z - 1, L))];
+    int8_t *si = &o->s[orc_idx(o, x, y, z)];
+    int dE = 2 * (int)(*si) * h;
+    if (dE < 0) {
+        *si = (int8_t)(-*si);
+    } else if (dE == 0) {
+        if (orc_site_bit(o->seed, L, x, y, z, t, 0u)) *si = (int8_t)(-*si);
+    }
+}
+
+/* D7 half-sweep: every site of colour c = (x+y+z) mod 2 is
+ * proposed exactly once; neighbours all have the other colour and are frozen.
+ * order: 0 = lexicographic (z,y,x), 1 = reverse lexicographic,
+ *        2 = a seeded random permutation of the sites (small L; pin P6).   */
+void orc_half_sweep(orc_t *o, uint32_t t, int c, int order, uint64_t order_seed)
+{
+    const int L = o->L;
+    if (order == 0) {
+        /* same-colour sites do not interact, so planes can go
+         * in parallel without changing any result (checked by pin P6). */
+        #pragma omp parallel for schedule(static)
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x)
+                    if (((x + y + z) & 1) == c) orc_update_site(o, x, y, z, t);
+    } else if (order == 1) {
+        for (int z = L - 1; z >= 0; --z)
+            for (int y = L - 1; y >= 0; --y)
+                for (int x = L - 1; x >= 0; --x)
+                    if (((x + y + z) & 1) == c) orc_update_site(o, x, y, z, t);
+    } else {
+        size_t N = (size_t)L * L * L;
+        uint32_t *perm = (uint32_t *)malloc(N * sizeof(uint32_t));
+        for (size_t i = 0; i < N; ++i) perm[i] = (uint32_t)i;
+        uint64_t st = order_seed * 6364136223846793005ull + 1442695040888963407ull;
+        for (size_t i = N - 1; i > 0; --i) {           /* Fisher-Yates */
+            st = st * 6364136223846793005ull + 1442695040888963407ull;
+            size_t j = (size_t)((st >> 33) % (uint64_t)(i + 1));
+            uint32_t tmp = perm[i]; perm[i] = perm[j]; perm[j] = tmp;
+        }
+        for (size_t i = 0; i < N; ++i) {
+            int x = (int)(perm[i] % (uint32_t)L);
+            int y = (int)((perm[i] / (uint32_t)L) % (uint32_t)L);
+            int z = (int)(perm[i] / ((uint32_t)L * (uint32_t)L));
+            if (((x + y + z) & 1) == c) orc_update_site(o, x, y, z, t);
+        }
+        free(perm);
+    }
+}
+
+/* D7 sweep = "01 cycle": colour 0 fully, then colour 1
+ * (which sees the updated colour 0).  One sweep = N proposals = 1 MCS.     */
+void orc_sweep(orc_t *o, uint64_t n_sweeps)
+{
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        orc_half_sweep(o, o->sweep, 0, 0, 0);
+        orc_half_sweep(o, o->sweep, 1, 0, 0);
+        o->sweep += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* Brute-force variant for tiny L (pin P7): Delta E is obtained as     */
+/* H(flipped configuration) - H(configuration), H = -sum over all 3N   */
+/* bonds of s_i s_j (each bond once: +x, +y, +z neighbour of each site).*/
+/* ------------------------------------------------------------------ */
+int64_t orc_energy(const orc_t *o)
+{
+    const int L = o->L;
+    int64_t H = 0;
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                int s = o->s[orc_idx(o, x, y, z)];
+                H -= s * o->s[orc_idx(o, orc_mod(x + 1, L), y, z)];
+                H -= s * o->s[orc_idx(o, x, orc_mod(y + 1, L), z)];
+                H -= s * o->s[orc_idx(o, x, y, orc_mod(z + 1, L))];
+            }
+    return H;
+}
+
+void orc_half_sweep_brute(orc_t *o, uint32_t t, int c)
+{
+    const int L = o->L;
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                if (((x + y + z) & 1) != c) continue;
+                int8_t *si = &o->s[orc_idx(o, x, y, z)];
+                int64_t H0 = orc_energy(o);
+                *si = (int8_t)(-*si);
+                int64_t H1 = orc_energy(o);
+                int64_t dE = H1 - H0;
+                int accept;
+                if (dE < 0) accept = 1;
+                else if (dE > 0) accept = 0;
+                else accept = orc_site_bit(o->seed, L, x, y, z, t, 0u);
+                if (!accept) *si = (int8_t)(-*si);
+            }
+}
+
+void orc_sweep_brute(orc_t *o, uint64_t n_sweeps)
+{
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        orc_half_sweep_brute(o, o->sweep, 0);
+        orc_half_sweep_brute(o, o->sweep, 1);
+        o->sweep += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* D8 integer measurements.                                            */
+/*   N_up = #{s = +1};                                                 */
+/*   A_mu(r) = #{sites i : s_i != s_{i + r e_mu}}, mu = x,y,z, over    */
+/*   ALL N sites i, periodic (eq. (2) PAPER.md:43 reduced to counts:   */
+/*   s_i s_j = +1 / -1 for parallel / antiparallel pairs).             */
+/* r_list[n_r] are the displacements wanted (0 <= r <= L/2);           */
+/* antipar is [3][n_r], row-major, same order as r_list.               */
+/* ------------------------------------------------------------------ */
+void orc_measure(const orc_t *o, const int32_t *r_list, int n_r,
+                 uint64_t *n_up, uint64_t *antipar)
+{
+    const int L = o->L;
+    uint64_t up = 0;
+    #pragma omp parallel for schedule(static) reduction(+:up)
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x)
+                if (o->s[orc_idx(o, x, y, z)] == 1) up += 1;
+    *n_up = up;
+
+    for (int ir = 0; ir < n_r; ++ir) {
+        const int r = r_list[ir];
+        uint64_t ax = 0, ay = 0, az = 0;
+        #pragma omp parallel for schedule(static) reduction(+:ax,ay,az)
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    int8_t s = o->s[orc_idx(o, x, y, z)];
+                    if (s != o->s[orc_idx(o, orc_mod(x + r, L), y, z)]) ax += 1;
+                    if (s != o->s[orc_idx(o, x, orc_mod(y + r, L), z)]) ay += 1;
+                    if (s != o->s[orc_idx(o, x, y, orc_mod(z + r, L))]) az += 1;
+                }
+        antipar[0 * (size_t)n_r + ir] = ax;
+        antipar[1 * (size_t)n_r + ir] = ay;
+        antipar[2 * (size_t)n_r + ir] = az;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* D9 fp64 post-processing of the counts, in exactly this order:       */
+/*   m = (double)(2 N_up - N) / (double)N;                             */
+/*   S(r) = 3N - 2 (A_x + A_y + A_z)(r)           (int64);             */
+/*   C(r) = (double)S(r) / (double)(3N) - m*m     (eq. 2; */
+/*          lattice average of one configuration, axis-averaged);      */
+/*   ell: r0 = smallest r in [0, L/2-1] with C(r0) >= c > C(r0+1);     */
+/*        ell = r0 + (C(r0) - c) / (C(r0) - C(r0+1))  (PAPER.md:51,    */
+/*        linear interpolation); NaN if there is no such r0.           */
+/* antipar is [3][L/2+1] here (all displacements).                     */
+/* ------------------------------------------------------------------ */
+void orc_postprocess(int L, uint64_t n_up, const uint64_t *antipar, double c_intercept,
+                     double *m_out, double *C, double *ell)
+{
+    const int nr = L / 2 + 1;
+    const int64_t N = (int64_t)L * L * L;
+    double m = (double)(2 * (int64_t)n_up - N) / (double)N;
+    *m_out = m;
+    for (int r = 0; r < nr; ++r) {
+        int64_t A = (int64_t)antipar[0 * nr + r] + (int64_t)antipar[1 * nr + r]
+                  + (int64_t)antipar[2 * nr + r];
+        int64_t S = 3 * N - 2 * A;
+        C[r] = (double)S / (double)(3 * N) - m * m;
+    }
+    *ell = NAN;
+    for (int r = 0; r + 1 < nr; ++r) {
+        if (C[r] >= c_intercept && C[r + 1] < c_intercept) {
+            *ell = (double)r + (C[r] - c_intercept) / (C[r] - C[r + 1]);
+            break;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* D3 export / import: colour 0 words then colour 1 words; 32-bit      */
+/* words, bit j (LSB = 0) of word w holds bit index b = 32 w + j;      */
+/* bit value 1 <=> s = +1.                                             */
+/* words per colour = ceil(L^3/2 / 32).                                */
+/* ------------------------------------------------------------------ */
+size_t orc_words_per_colour(int L)
+{
+    uint64_t bits = (uint64_t)L * L * L / 2;
+    return (size_t)((bits + 31) / 32);
+}
+
+void orc_export(const orc_t *o, uint32_t *words)
+{
+    const int L = o->L;
+    size_t wpc = orc_words_per_colour(L);
+    memset(words, 0, 2 * wpc * sizeof(uint32_t));
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                int c = (x + y + z) & 1;
+                uint64_t b = orc_bit_index(L, x, y, z);
+                if (o->s[orc_idx(o, x, y, z)] == 1)
+                    words[(size_t)c * wpc + (size_t)(b >> 5)] |= (1u << (b & 31));
+            }
+}
+
+void orc_import(orc_t *o, const uint32_t *words, uint32_t sweep)
+{
+    const int L = o->L;
+    size_t wpc = orc_words_per_colour(L);
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                int c = (x + y + z) & 1;
+                uint64_t b = orc_bit_index(L, x, y, z);
+                uint32_t bit = (words[(size_t)c * wpc + (size_t)(b >> 5)] >> (b & 31)) & 1u;
+                o->s[orc_idx(o, x, y, z)] = bit ? (int8_t)1 : (int8_t)-1;
+            }
+    o->sweep = sweep;
+}
+
+/* how many threads the OpenMP loops above use (bench.py reports it) */
+#ifdef _OPENMP
+#include <omp.h>
+int orc_num_threads(void) { return omp_get_max_threads(); }
+void orc_set_num_threads(int n) { omp_set_num_threads(n); }
+#else
+int orc_num_threads(void) { return 1; }
+void orc_set_num_threads(int n) { (void)n; }
+#endif

@@ -1,0 +1,231 @@
+"""ctypes front end of the CPU oracle (oracle/ising_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+and bench.py's cpu_baseline / --impl reference leg may import this module.
+It imports nothing from paper_2305_12161_b200 and the CUDA path imports
+nothing from here.
+
+What each call computes and which passage of the paper it follows is stated in
+ising_oracle.c next to the function of the same name (eq. (6),
+PAPER.md:116 sweep order, eq. (2), PAPER.md:51 ell).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "ising_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile ising_oracle.c with gcc (-O2, OpenMP over z-planes only)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + ".tmp.%d" % os.getpid()
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+    subprocess.check_call(cmd)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        l = C.CDLL(build())
+        u32p = C.POINTER(C.c_uint32)
+        u64p = C.POINTER(C.c_uint64)
+        i32p = C.POINTER(C.c_int32)
+        dp = C.POINTER(C.c_double)
+        l.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
+        l.orc_philox4x32_10.restype = None
+        l.orc_create.argtypes = [C.c_int, C.c_uint64]
+        l.orc_create.restype = C.c_void_p
+        l.orc_free.argtypes = [C.c_void_p]
+        l.orc_free.restype = None
+        l.orc_spins.argtypes = [C.c_void_p]
+        l.orc_spins.restype = C.POINTER(C.c_int8)
+        l.orc_get_sweep.argtypes = [C.c_void_p]
+        l.orc_get_sweep.restype = C.c_uint32
+        l.orc_set_sweep.argtypes = [C.c_void_p, C.c_uint32]
+        l.orc_set_sweep.restype = None
+        l.orc_set_seed.argtypes = [C.c_void_p, C.c_uint64]
+        l.orc_set_seed.restype = None
+        l.orc_site_bit.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int,
+                                   C.c_uint32, C.c_uint32]
+        l.orc_site_bit.restype = C.c_int
+        l.orc_init_random.argtypes = [C.c_void_p]
+        l.orc_init_random.restype = None
+        l.orc_half_sweep.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_int, C.c_uint64]
+        l.orc_half_sweep.restype = None
+        l.orc_sweep.argtypes = [C.c_void_p, C.c_uint64]
+        l.orc_sweep.restype = None
+        l.orc_energy.argtypes = [C.c_void_p]
+        l.orc_energy.restype = C.c_int64
+        l.orc_half_sweep_brute.argtypes = [C.c_void_p, C.c_uint32, C.c_int]
+        l.orc_half_sweep_brute.restype = None
+        l.orc_sweep_brute.argtypes = [C.c_void_p, C.c_uint64]
+        l.orc_sweep_brute.restype = None
+        l.orc_measure.argtypes = [C.c_void_p, i32p, C.c_int, u64p, u64p]
+        l.orc_measure.restype = None
+        l.orc_postprocess.argtypes = [C.c_int, C.c_uint64, u64p, C.c_double, dp, dp, dp]
+        l.orc_postprocess.restype = None
+        l.orc_words_per_colour.argtypes = [C.c_int]
+        l.orc_words_per_colour.restype = C.c_size_t
+        l.orc_export.argtypes = [C.c_void_p, u32p]
+        l.orc_export.restype = None
+        l.orc_import.argtypes = [C.c_void_p, u32p, C.c_uint32]
+        l.orc_import.restype = None
+        l.orc_num_threads.argtypes = []
+        l.orc_num_threads.restype = C.c_int
+        l.orc_set_num_threads.argtypes = [C.c_int]
+        l.orc_set_num_threads.restype = None
+        _lib = l
+    return _lib
+
+
+def _p(a, ty):
+    return a.ctypes.data_as(C.POINTER(ty))
+
+
+def philox4x32_10(ctr, key):
+    """D5.  ctr: 4 uint32, key: 2 uint32 -> 4 uint32 (numpy)."""
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib().orc_philox4x32_10(_p(c, C.c_uint32), _p(k, C.c_uint32), _p(out, C.c_uint32))
+    return out
+
+
+def site_bit(seed, L, x, y, z, t, tag):
+    return int(lib().orc_site_bit(int(seed), L, x, y, z, t, tag))
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(int(n))
+
+
+def postprocess(L, n_up, antipar, c_intercept=0.5):
+    """D9.  antipar: uint64 [3][L/2+1].  Returns (m, C[L/2+1], ell)."""
+    nr = L // 2 + 1
+    a = np.ascontiguousarray(antipar, dtype=np.uint64).reshape(3, nr)
+    Cr = np.zeros(nr, dtype=np.float64)
+    m = C.c_double()
+    ell = C.c_double()
+    lib().orc_postprocess(L, int(n_up), _p(a, C.c_uint64), float(c_intercept),
+                          C.byref(m), _p(Cr, C.c_double), C.byref(ell))
+    return m.value, Cr, ell.value
+
+
+class Oracle:
+    """One lattice of the CPU oracle (int8 per spin)."""
+
+    def __init__(self, L: int, seed: int, init: bool = True):
+        self._l = lib()
+        self.L = int(L)
+        self.seed = int(seed)
+        self._h = self._l.orc_create(self.L, self.seed)
+        if not self._h:
+            raise ValueError("oracle: L must be even and >= 4 (D1)")
+        if init:
+            self._l.orc_init_random(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._l.orc_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- state ---------------------------------------------------------
+    @property
+    def spins(self) -> np.ndarray:
+        """View [z][y][x] of the int8 spins (writable, no copy)."""
+        n = self.L ** 3
+        buf = (C.c_int8 * n).from_address(C.addressof(self._l.orc_spins(self._h).contents))
+        buf._owner = self          # the view keeps the lattice alive
+        return np.frombuffer(buf, dtype=np.int8).reshape(self.L, self.L, self.L)
+
+    @property
+    def sweep_count(self) -> int:
+        return int(self._l.orc_get_sweep(self._h))
+
+    @sweep_count.setter
+    def sweep_count(self, t: int):
+        self._l.orc_set_sweep(self._h, int(t))
+
+    def set_seed(self, seed: int):
+        self.seed = int(seed)
+        self._l.orc_set_seed(self._h, self.seed)
+
+    def init_random(self):
+        self._l.orc_init_random(self._h)
+
+    # -- dynamics ------------------------------------------------------
+    def half_sweep(self, t: int, c: int, order: int = 0, order_seed: int = 0):
+        self._l.orc_half_sweep(self._h, int(t), int(c), int(order), int(order_seed))
+
+    def sweep(self, n: int = 1):
+        self._l.orc_sweep(self._h, int(n))
+
+    def half_sweep_brute(self, t: int, c: int):
+        self._l.orc_half_sweep_brute(self._h, int(t), int(c))
+
+    def sweep_brute(self, n: int = 1):
+        self._l.orc_sweep_brute(self._h, int(n))
+
+    def energy(self) -> int:
+        return int(self._l.orc_energy(self._h))
+
+    # -- measurements --------------------------------------------------
+    def measure(self, r_list=None):
+        """D8.  Returns (n_up, antipar[3][len(r_list)]); r_list defaults to 0..L/2."""
+        if r_list is None:
+            r_list = np.arange(self.L // 2 + 1, dtype=np.int32)
+        r = np.ascontiguousarray(r_list, dtype=np.int32)
+        a = np.zeros((3, len(r)), dtype=np.uint64)
+        n_up = C.c_uint64()
+        self._l.orc_measure(self._h, _p(r, C.c_int32), len(r), C.byref(n_up), _p(a, C.c_uint64))
+        return int(n_up.value), a
+
+    def measure_full(self, c_intercept: float = 0.5):
+        """D8 + D9 over all r: dict with n_up, n_broken, antipar, m, C, ell."""
+        n_up, a = self.measure()
+        m, Cr, ell = postprocess(self.L, n_up, a, c_intercept)
+        return {"n_up": n_up, "n_broken": int(a[0, 1] + a[1, 1] + a[2, 1]),
+                "antipar": a, "m": m, "C": Cr, "ell": ell, "sweep": self.sweep_count}
+
+    # -- D3 packed layout ---------------------------------------------
+    def words_per_colour(self) -> int:
+        return int(self._l.orc_words_per_colour(self.L))
+
+    def export_words(self) -> np.ndarray:
+        w = np.zeros(2 * self.words_per_colour(), dtype=np.uint32)
+        self._l.orc_export(self._h, _p(w, C.c_uint32))
+        return w
+
+    def import_words(self, words, sweep: int):
+        w = np.ascontiguousarray(words, dtype=np.uint32)
+        assert w.size == 2 * self.words_per_colour()
+        self._l.orc_import(self._h, _p(w, C.c_uint32), int(sweep))
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))

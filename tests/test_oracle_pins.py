@@ -1,0 +1,505 @@
+"""Pins of the CPU oracle (oracle/ising_oracle.c) against what the paper and the
+mathematics fix -- none of them against the CUDA path.  SURVEY.md 8(c) P1..P11.
+
+Each pin is chosen so that a plausible mistake in the oracle (a dropped term,
+a wrong sign or index, a transposed axis, a wrong Philox round) fails it.
+"""
+import math
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2305_12161_b200 import inputs
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+MASK = 0xFFFFFFFF
+
+
+def py_philox(ctr, key):
+    """Big-integer restatement of Philox4x32-10 written from D5 (P1-ii)."""
+    c = [int(v) for v in ctr]
+    k = [int(v) for v in key]
+    for rnd in range(10):
+        if rnd:
+            k = [(k[0] + W0) & MASK, (k[1] + W1) & MASK]
+        p0 = M0 * c[0]
+        p1 = M1 * c[2]
+        c = [((p1 >> 32) ^ c[1] ^ k[0]) & MASK, p1 & MASK,
+             ((p0 >> 32) ^ c[3] ^ k[1]) & MASK, p0 & MASK]
+    return c
+
+
+def py_site_bit(seed, L, x, y, z, t, tag):
+    """D3 + D5 addressing restated in Python."""
+    c = (x + y + z) & 1
+    b = (z * L + y) * (L // 2) + (x >> 1)
+    out = py_philox([b >> 7, t, c, tag], [seed & MASK, seed >> 32])
+    return (out[(b >> 5) & 3] >> (b & 31)) & 1
+
+
+# ---------------------------------------------------------------- P1: Philox
+def test_philox_known_answers(golden_dir):
+    n = 0
+    for line in open(os.path.join(golden_dir, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or "->" not in line:
+            continue
+        lhs, rhs = line.split("->")
+        v = [int(t, 16) for t in lhs.split()]
+        want = [int(t, 16) for t in rhs.split()]
+        got = [int(g) for g in orc.philox4x32_10(v[:4], v[4:])]
+        assert got == want
+        assert py_philox(v[:4], v[4:]) == want
+        n += 1
+    assert n == 3
+
+
+def test_philox_vs_python_restatement():
+    rng = np.random.Generator(np.random.PCG64(7))
+    for _ in range(2000):
+        v = [int(t) for t in rng.integers(0, 2 ** 32, size=6, dtype=np.uint64)]
+        assert [int(g) for g in orc.philox4x32_10(v[:4], v[4:])] == py_philox(v[:4], v[4:])
+
+
+@pytest.mark.skipif(shutil.which("nvcc") is None, reason="nvcc not on PATH")
+def test_philox_vs_curand_host(tmp_path):
+    """NVIDIA's curand_Philox4x32_10 (toolkit header, host path) on 20000 random inputs."""
+    exe = str(tmp_path / "curand_philox_host")
+    subprocess.check_call(["nvcc", "-O1", "-Wno-deprecated-gpu-targets", "-o", exe,
+                           os.path.join(HERE, "pins", "curand_philox_host.cu")],
+                          stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL)
+    rng = np.random.Generator(np.random.PCG64(11))
+    vals = rng.integers(0, 2 ** 32, size=(20000, 6), dtype=np.uint64)
+    # structured counters as the method uses them: (q, t, c, tag)
+    vals[:5000, 1] = np.arange(5000)
+    vals[:5000, 2] = np.arange(5000) & 1
+    vals[:5000, 3] = (np.arange(5000) >> 1) & 1
+    txt = "\n".join(" ".join("%x" % int(t) for t in row) for row in vals) + "\n"
+    out = subprocess.run([exe], input=txt, capture_output=True, text=True, check=True).stdout
+    lines = out.strip().split("\n")
+    assert len(lines) == len(vals)
+    for row, line in zip(vals, lines):
+        want = [int(t, 16) for t in line.split()]
+        got = [int(g) for g in orc.philox4x32_10(row[:4], row[4:])]
+        assert got == want
+
+
+def test_site_bit_addressing():
+    """D3/D5: which Philox word and bit a site reads (P1 + layout)."""
+    rng = np.random.Generator(np.random.PCG64(3))
+    for L in (4, 6, 8, 64, 128):
+        for _ in range(300):
+            x, y, z = (int(v) for v in rng.integers(0, L, size=3))
+            t = int(rng.integers(0, 2 ** 32 - 1))
+            tag = int(rng.integers(0, 2))
+            seed = int(rng.integers(0, 2 ** 63)) * 2 + int(rng.integers(0, 2))
+            assert orc.site_bit(seed, L, x, y, z, t, tag) == py_site_bit(seed, L, x, y, z, t, tag)
+
+
+# ---------------------------------------------------------------- P2: site rule
+def _find_t_with_bit(seed, L, x, y, z, want):
+    for t in range(1000):
+        if py_site_bit(seed, L, x, y, z, t, 0) == want:
+            return t
+    raise AssertionError
+
+
+def test_site_rule_exhaustive():
+    """All 2^6 neighbour configurations x own spin x tie bit: outcome of the oracle ==
+    eq. (6) in three independent forms (Delta-E, antiparallel count, majority vote)."""
+    L, seed = 4, 12345
+    x, y, z = 1, 2, 3
+    c = (x + y + z) & 1
+    nbrs = [((x + 1) % L, y, z), ((x - 1) % L, y, z), (x, (y + 1) % L, z),
+            (x, (y - 1) % L, z), (x, y, (z + 1) % L), (x, y, (z - 1) % L)]
+    t_for = {0: _find_t_with_bit(seed, L, x, y, z, 0), 1: _find_t_with_bit(seed, L, x, y, z, 1)}
+    o = orc.Oracle(L, seed, init=False)
+    rng = np.random.Generator(np.random.PCG64(5))
+    cases = 0
+    for cfg in range(64):
+        for own in (-1, 1):
+            for rho in (0, 1):
+                s = o.spins
+                s[...] = np.where(rng.random((L, L, L)) < 0.5, 1, -1)
+                nb = [1 if (cfg >> i) & 1 else -1 for i in range(6)]
+                for (nx, ny, nz), v in zip(nbrs, nb):
+                    s[nz, ny, nx] = v
+                s[z, y, x] = own
+                o.half_sweep(t_for[rho], c)
+                got = int(o.spins[z, y, x])
+                # form 1: eq. (6) with Delta E = 2 s_i sum s_j
+                dE = 2 * own * sum(nb)
+                f1 = -own if dE < 0 else (own if dE > 0 else (-own if rho else own))
+                # form 2: n antiparallel neighbours: n>=4 flip, n==3 flip iff rho, n<=2 keep
+                n = sum(1 for v in nb if v != own)
+                f2 = -own if n >= 4 else ((-own if rho else own) if n == 3 else own)
+                # form 3: majority vote of the neighbours, own^rho on a 3-3 split
+                up = sum(1 for v in nb if v == 1)
+                f3 = 1 if up >= 4 else (-1 if up <= 2 else (-own if rho else own))
+                assert f1 == f2 == f3
+                assert got == f1, (cfg, own, rho)
+                # neighbours (other colour) are untouched by this half-sweep
+                for (nx, ny, nz), v in zip(nbrs, nb):
+                    assert int(o.spins[nz, ny, nx]) == v
+                cases += 1
+    assert cases == 256
+
+
+# ---------------------------------------------------------------- P3: energy
+def _n_broken(o):
+    _, a = o.measure([1])
+    return int(a[:, 0].sum())
+
+
+def test_energy_never_increases_per_half_sweep():
+    L = 16
+    N = L ** 3
+    o = orc.Oracle(L, 99)
+    prev = _n_broken(o)
+    assert o.energy() == -3 * N + 2 * prev          # E = -3N + 2B
+    strictly = 0
+    for t in range(25):
+        for c in (0, 1):
+            o.half_sweep(t, c)
+            cur = _n_broken(o)
+            assert cur <= prev
+            assert o.energy() == -3 * N + 2 * cur
+            strictly += cur < prev
+            prev = cur
+    assert strictly > 5
+
+
+# ---------------------------------------------------------------- P4: fixed points
+@pytest.mark.parametrize("seed", [0, 1, 2 ** 63 + 5])
+def test_fixed_points(seed):
+    L = 8
+    states = [inputs.all_up(L), -inputs.all_up(L)]
+    for axis in (0, 1, 2):
+        states.append(inputs.slab(L, axis, 3, 3))       # flat interfaces: n = 1 there
+        states.append(inputs.slab(L, axis, L - 1, 2))   # slab across the periodic wrap
+    for s0 in states:
+        o = orc.Oracle(L, seed, init=False)
+        o.spins[...] = s0
+        o.sweep(3)
+        assert np.array_equal(o.spins, s0)
+
+
+# ---------------------------------------------------------------- P5: closed forms
+def test_neel_state_orders_in_one_half_sweep():
+    L = 8
+    o = orc.Oracle(L, 4, init=False)
+    o.spins[...] = inputs.neel(L)           # black +1, white -1: every bond broken
+    assert _n_broken(o) == 3 * L ** 3
+    o.half_sweep(0, 0)                      # every black site has n = 6 -> flips
+    assert np.all(o.spins == -1)
+    assert _n_broken(o) == 0
+    # and the other way round: updating white first orders with the black value
+    o.spins[...] = inputs.neel(L)
+    o.half_sweep(0, 1)
+    assert np.all(o.spins == 1)
+
+
+def test_single_reversed_spin_disappears():
+    L = 8
+    for (x, y, z) in [(0, 0, 0), (7, 7, 7), (3, 4, 0), (1, 0, 0)]:
+        c = (x + y + z) & 1
+        o = orc.Oracle(L, 4, init=False)
+        o.spins[...] = inputs.single_spin(L, x, y, z)
+        assert _n_broken(o) == 6
+        o.half_sweep(0, 1 - c)              # wrong colour: its neighbours have n = 1, stay
+        assert np.array_equal(o.spins, inputs.single_spin(L, x, y, z))
+        o.half_sweep(0, c)                  # n = 6 -> flips
+        assert np.all(o.spins == 1)
+
+
+@pytest.mark.parametrize("corner", [(2, 2, 2), (7, 3, 3), (3, 7, 3), (3, 3, 7), (7, 7, 7), (0, 5, 7)])
+def test_cube_ties_follow_their_own_philox_bit(corner):
+    """2x2x2 reversed cube: in half-sweep (t,0) its 4 black sites have n = 3 and flip iff
+    their own bit is 1; every other black site has n <= 1 and stays (P5)."""
+    L, seed = 8, 2024
+    x0, y0, z0 = corner
+    for t in (0, 1, 17):
+        s0 = inputs.cube(L, x0, y0, z0)
+        o = orc.Oracle(L, seed, init=False)
+        o.spins[...] = s0
+        o.half_sweep(t, 0)
+        want = s0.copy()
+        for dz in range(2):
+            for dy in range(2):
+                for dx in range(2):
+                    x, y, z = (x0 + dx) % L, (y0 + dy) % L, (z0 + dz) % L
+                    if (x + y + z) % 2 == 0 and py_site_bit(seed, L, x, y, z, t, 0):
+                        want[z, y, x] = 1
+        assert np.array_equal(o.spins, want)
+
+
+# ---------------------------------------------------------------- P6: order independence
+@pytest.mark.parametrize("L", [6, 8, 12])
+def test_half_sweep_is_order_independent(L):
+    base = orc.Oracle(L, 31)
+    s0 = base.spins.copy()
+    for t in range(3):
+        for c in (0, 1):
+            results = []
+            for order, oseed in [(0, 0), (1, 0), (2, 1), (2, 2)]:
+                o = orc.Oracle(L, 31, init=False)
+                o.spins[...] = s0
+                o.half_sweep(t, c, order, oseed)
+                results.append(o.spins.copy())
+            for r in results[1:]:
+                assert np.array_equal(results[0], r)
+            s0 = results[0]
+
+
+# ---------------------------------------------------------------- P7: brute force
+@pytest.mark.parametrize("L,n_seeds,n_sweeps", [(4, 100, 20), (6, 12, 10), (8, 3, 6)])
+def test_brute_force_energy_difference(L, n_seeds, n_sweeps):
+    """Delta E as H(flipped) - H(config) over all 3N bonds vs the local-field form."""
+    for seed in range(n_seeds):
+        a = orc.Oracle(L, seed)
+        b = orc.Oracle(L, seed)
+        assert np.array_equal(a.spins, b.spins)
+        for _ in range(n_sweeps):
+            a.sweep(1)
+            b.sweep_brute(1)
+            assert np.array_equal(a.spins, b.spins)
+        assert a.sweep_count == b.sweep_count == n_sweeps
+
+
+def test_python_reference_sweep_L4():
+    """An independent pure-Python site loop (own Philox, own indexing) on L=4 and L=6."""
+    for L, seed in [(4, 5), (4, 6), (6, 7)]:
+        o = orc.Oracle(L, seed)
+        s = np.zeros((L, L, L), dtype=np.int64)
+        for z in range(L):
+            for y in range(L):
+                for x in range(L):
+                    s[z, y, x] = 1 if py_site_bit(seed, L, x, y, z, 0, 1) else -1
+        assert np.array_equal(o.spins, s)
+        for t in range(6):
+            for c in (0, 1):
+                for z in range(L):
+                    for y in range(L):
+                        for x in range(L):
+                            if (x + y + z) % 2 != c:
+                                continue
+                            h = (s[z, y, (x + 1) % L] + s[z, y, (x - 1) % L] + s[z, (y + 1) % L, x]
+                                 + s[z, (y - 1) % L, x] + s[(z + 1) % L, y, x] + s[(z - 1) % L, y, x])
+                            dE = 2 * s[z, y, x] * h
+                            if dE < 0 or (dE == 0 and py_site_bit(seed, L, x, y, z, t, 0)):
+                                s[z, y, x] = -s[z, y, x]
+            o.sweep(1)
+            assert np.array_equal(o.spins, s)
+
+
+# ---------------------------------------------------------------- P8/P9: statistics
+def test_start_statistics_and_first_half_sweep():
+    L, seed = 64, 1
+    N = L ** 3
+    o = orc.Oracle(L, seed)
+    n_up, a = o.measure([1, 2, 7, 32])
+    assert abs(n_up - N / 2) < 4 * 0.5 * math.sqrt(N)                     # m ~ 0
+    for mu in range(3):
+        for i in range(4):
+            assert abs(int(a[mu, i]) - N / 2) < 5 * 0.5 * math.sqrt(N)   # no correlations at T=inf
+    nb = int(a[:, 0].sum())
+    assert abs(nb - 1.5 * N) < 5 * 0.5 * math.sqrt(3 * N)
+    # ties among black sites: P(n = 3) = 20/64; flips among ties ~ 1/2
+    s = o.spins.astype(np.int64)
+    h = sum(np.roll(s, sh, axis=ax) for ax in range(3) for sh in (1, -1))
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    black = ((x + y + z) & 1) == 0
+    ties = black & (h == 0)
+    n_ties = int(ties.sum())
+    assert abs(n_ties - (N / 2) * 20 / 64) < 5 * math.sqrt((N / 2) * (20 / 64) * (44 / 64))
+    before = o.spins.copy()
+    o.half_sweep(0, 0)
+    flipped = before != o.spins
+    assert not np.any(flipped & ~black)
+    n_tie_flips = int((flipped & ties).sum())
+    assert abs(n_tie_flips - n_ties / 2) < 5 * 0.5 * math.sqrt(n_ties)
+    # P9: E[n_broken after the first black half-sweep] = (N/2) * 132/64
+    nb1 = _n_broken(o)
+    assert abs(nb1 - 1.03125 * N) < 0.005 * 1.03125 * N
+    # flipped fraction of colour 0: P(n>=4) + P(n=3)/2 = 22/64 + 10/64 = 1/2
+    assert abs(int(flipped.sum()) - N / 4) < 5 * 0.5 * math.sqrt(N / 2)
+
+
+def test_seeds_and_tags_are_separated():
+    """tag 1 (start) and tag 0 (ties of sweep 0) draw different bits; seeds differ."""
+    L = 8
+    a = orc.Oracle(L, 1).spins.copy()
+    b = orc.Oracle(L, 2).spins.copy()
+    c = orc.Oracle(L, 1 << 32).spins.copy()      # high half of the seed is part of the key
+    assert 0.3 < np.mean(a != b) < 0.7
+    assert 0.3 < np.mean(a != c) < 0.7
+    start_bits = np.array([[[py_site_bit(1, L, x, y, z, 0, 1) for x in range(L)]
+                            for y in range(L)] for z in range(L)])
+    tie_bits = np.array([[[py_site_bit(1, L, x, y, z, 0, 0) for x in range(L)]
+                          for y in range(L)] for z in range(L)])
+    assert np.array_equal(start_bits == 1, a == 1)
+    assert 0.3 < np.mean(start_bits != tie_bits) < 0.7
+
+
+# ---------------------------------------------------------------- P10: measurements
+def _np_measure(s, r_list):
+    """numpy restatement of D8 with np.roll (a library routine)."""
+    n_up = int((s == 1).sum())
+    a = np.zeros((3, len(r_list)), dtype=np.uint64)
+    for i, r in enumerate(r_list):
+        a[0, i] = int((s != np.roll(s, -r, axis=2)).sum())   # x is the last index
+        a[1, i] = int((s != np.roll(s, -r, axis=1)).sum())
+        a[2, i] = int((s != np.roll(s, -r, axis=0)).sum())
+    return n_up, a
+
+
+def test_measure_vs_numpy_and_identities():
+    L = 12
+    o = orc.Oracle(L, 8)
+    o.sweep(2)
+    s = o.spins.copy()
+    rl = list(range(L // 2 + 1))
+    n_up, a = o.measure()
+    n_up2, a2 = _np_measure(s, rl)
+    assert n_up == n_up2 and np.array_equal(a, a2)
+    assert np.all(a[:, 0] == 0)
+    assert o.measure_full()["n_broken"] == int(a[:, 1].sum())
+    # translation invariance
+    for shift in [(1, 0, 0), (0, 5, 0), (3, 2, 7)]:
+        o2 = orc.Oracle(L, 0, init=False)
+        o2.spins[...] = np.roll(s, shift, axis=(0, 1, 2))
+        n2, b = o2.measure()
+        assert n2 == n_up and np.array_equal(a, b)
+    # axis permutation: spins'[z][y][x] = s[x][y][z] swaps the x and z rows
+    o3 = orc.Oracle(L, 0, init=False)
+    o3.spins[...] = np.transpose(s, (2, 1, 0))
+    _, b = o3.measure()
+    assert np.array_equal(b[0], a[2]) and np.array_equal(b[2], a[0]) and np.array_equal(b[1], a[1])
+    o4 = orc.Oracle(L, 0, init=False)
+    o4.spins[...] = np.transpose(s, (0, 2, 1))             # swaps x and y
+    _, b = o4.measure()
+    assert np.array_equal(b[0], a[1]) and np.array_equal(b[1], a[0]) and np.array_equal(b[2], a[2])
+    # global flip changes N_up -> N - N_up and no pair count
+    o5 = orc.Oracle(L, 0, init=False)
+    o5.spins[...] = -s
+    n5, b = o5.measure()
+    assert n5 == L ** 3 - n_up and np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_measure_slab_closed_form(axis):
+    """Slab of thickness L/2 normal to `axis`: A_axis(r) = 2 r L^2 (r <= L/2), others 0;
+    m = 0; C(r) = 1 - 4r/(3L); ell = 3L/8 exactly (linear C)."""
+    L = 16
+    o = orc.Oracle(L, 0, init=False)
+    o.spins[...] = inputs.slab(L, axis, 5, L // 2)
+    r = o.measure_full()
+    assert r["n_up"] == L ** 3 // 2
+    for mu in range(3):
+        for rr in range(L // 2 + 1):
+            assert int(r["antipar"][mu, rr]) == (2 * rr * L * L if mu == axis else 0)
+    assert r["m"] == 0.0
+    for rr in range(L // 2 + 1):
+        assert abs(r["C"][rr] - (1 - 4 * rr / (3 * L))) < 1e-15
+    assert abs(r["ell"] - 3 * L / 8) < 1e-12
+    assert r["n_broken"] == 2 * L * L
+
+
+def test_measure_all_up():
+    L = 8
+    o = orc.Oracle(L, 0, init=False)
+    o.spins[...] = inputs.all_up(L)
+    r = o.measure_full()
+    assert r["n_up"] == L ** 3 and r["n_broken"] == 0 and not r["antipar"].any()
+    assert np.all(r["C"] == 0.0) and math.isnan(r["ell"]) and r["m"] == 1.0
+
+
+def test_postprocess_worked_examples(golden_dir):
+    n = 0
+    for line in open(os.path.join(golden_dir, "postprocess_worked.txt")):
+        if line.startswith("#") or "|" not in line:
+            continue
+        f = [t.strip() for t in line.split("|")]
+        n_up = int(f[0])
+        A = [int(t) for t in f[1].split()]
+        c = float(f[2])
+        m_want = float(f[3])
+        C_want = [float(t) for t in f[4].split()]
+        ell_want = float(f[5])
+        # put the whole count on one axis: only the sum over axes enters D9
+        for axis in range(3):
+            a = np.zeros((3, 3), dtype=np.uint64)
+            a[axis] = A
+            m, Cr, ell = orc.postprocess(4, n_up, a, c)
+            assert m == m_want
+            assert np.allclose(Cr, C_want, rtol=0, atol=1e-15)
+            if math.isnan(ell_want):
+                assert math.isnan(ell)
+            else:
+                assert abs(ell - ell_want) < 1e-14
+        n += 1
+    assert n == 5
+
+
+# ---------------------------------------------------------------- P11 / D3
+def test_export_matches_independent_packer_and_roundtrip():
+    for L in (4, 6, 8, 64):
+        o = orc.Oracle(L, 21)
+        if L <= 8:
+            o.sweep(2)
+        w = o.export_words()
+        assert w.dtype == np.uint32 and w.size == 2 * inputs.words_per_colour(L)
+        assert np.array_equal(w, inputs.pack_spins(o.spins))
+        assert np.array_equal(inputs.unpack_words(w, L), o.spins)
+        o2 = orc.Oracle(L, 21, init=False)
+        o2.import_words(w, o.sweep_count)
+        assert np.array_equal(o2.spins, o.spins) and o2.sweep_count == o.sweep_count
+    # a single site lands on the documented word/bit (D3): L=64, site (x,y,z)=(5,2,1)
+    L = 64
+    s = -np.ones((L, L, L), dtype=np.int8)
+    s[1, 2, 5] = 1
+    o = orc.Oracle(L, 0, init=False)
+    o.spins[...] = s
+    w = o.export_words()
+    c = (5 + 2 + 1) & 1
+    b = (1 * L + 2) * (L // 2) + (5 >> 1)
+    wpc = L ** 3 // 64
+    assert int(w[c * wpc + (b >> 5)]) == 1 << (b & 31)
+    assert int(np.count_nonzero(w)) == 1
+
+
+def test_checkpoint_resume_is_exact():
+    L = 16
+    a = orc.Oracle(L, 77)
+    a.sweep(9)
+    b = orc.Oracle(L, 77)
+    b.sweep(4)
+    w = b.export_words()
+    c = orc.Oracle(L, 77, init=False)
+    c.import_words(w, 4)
+    c.sweep(5)
+    assert c.sweep_count == 9 and np.array_equal(a.spins, c.spins)
+    # the sweep index matters: resuming with a wrong counter gives another trajectory
+    d = orc.Oracle(L, 77, init=False)
+    d.import_words(w, 5)
+    d.sweep(5)
+    assert not np.array_equal(a.spins, d.spins)
+
+
+def test_threads_do_not_change_results():
+    L = 32
+    orc.set_num_threads(1)
+    a = orc.Oracle(L, 3)
+    a.sweep(4)
+    ra = a.measure_full()
+    orc.set_num_threads(max(2, os.cpu_count() or 2))
+    b = orc.Oracle(L, 3)
+    b.sweep(4)
+    rb = b.measure_full()
+    assert np.array_equal(a.spins, b.spins)
+    assert ra["n_up"] == rb["n_up"] and np.array_equal(ra["antipar"], rb["antipar"])
