@@ -31,6 +31,7 @@
  *                         permutation invariance, numpy restatement
  *   orc_postprocess     : closed forms, hand-worked example
  *   orc_export/import   : round trip, independent Python packer
+ *   orc_site_after      : equals orc_sweep site by site on small L
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -395,6 +396,43 @@ void orc_import(orc_t *o, const uint32_t *words, uint32_t sweep)
                 o->s[orc_idx(o, x, y, z)] = bit ? (int8_t)1 : (int8_t)-1;
             }
     o->sweep = sweep;
+}
+
+/* ------------------------------------------------------------------ */
+/* One site, computed one by one from the definition alone (no lattice */
+/* array): the value of site (x,y,z) after h half-sweeps from the      */
+/* T = infinity start of `seed`, by recursion over its light cone.     */
+/* Half-sweep number i = 1,2,... belongs to sweep t = (i-1)/2 and      */
+/* updates colour (i-1) mod 2 (D7).  Cost 7^h Philox calls: meant for  */
+/* sampled sites of lattices too large for the array version (L=2048). */
+/* Pinned against orc_sweep on small L (tests/test_oracle_pins.py).    */
+/* ------------------------------------------------------------------ */
+int orc_site_after(uint64_t seed, int L, int x, int y, int z, int h)
+{
+    if (h == 0) return orc_site_bit(seed, L, x, y, z, 0u, 1u) ? 1 : -1;
+    const int c = (x + y + z) & 1;
+    const int colour_updated = (h - 1) & 1;
+    const uint32_t t = (uint32_t)((h - 1) / 2);
+    const int s = orc_site_after(seed, L, x, y, z, h - 1);
+    if (colour_updated != c) return s;
+    const int sum = orc_site_after(seed, L, orc_mod(x + 1, L), y, z, h - 1)
+                  + orc_site_after(seed, L, orc_mod(x - 1, L), y, z, h - 1)
+                  + orc_site_after(seed, L, x, orc_mod(y + 1, L), z, h - 1)
+                  + orc_site_after(seed, L, x, orc_mod(y - 1, L), z, h - 1)
+                  + orc_site_after(seed, L, x, y, orc_mod(z + 1, L), h - 1)
+                  + orc_site_after(seed, L, x, y, orc_mod(z - 1, L), h - 1);
+    const int dE = 2 * s * sum;
+    if (dE < 0) return -s;
+    if (dE > 0) return s;
+    return orc_site_bit(seed, L, x, y, z, t, 0u) ? -s : s;
+}
+
+/* same for a list of sites, in parallel over the list */
+void orc_sites_after(uint64_t seed, int L, const int32_t *xyz, int n, int h, int8_t *out)
+{
+    #pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < n; ++i)
+        out[i] = (int8_t)orc_site_after(seed, L, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], h);
 }
 
 /* how many threads the OpenMP loops above use (bench.py reports it) */

@@ -85,6 +85,9 @@ def lib():
         l.orc_export.restype = None
         l.orc_import.argtypes = [C.c_void_p, u32p, C.c_uint32]
         l.orc_import.restype = None
+        l.orc_sites_after.argtypes = [C.c_uint64, C.c_int, i32p, C.c_int, C.c_int,
+                                      C.POINTER(C.c_int8)]
+        l.orc_sites_after.restype = None
         l.orc_num_threads.argtypes = []
         l.orc_num_threads.restype = C.c_int
         l.orc_set_num_threads.argtypes = [C.c_int]
@@ -108,6 +111,16 @@ def philox4x32_10(ctr, key):
 
 def site_bit(seed, L, x, y, z, t, tag):
     return int(lib().orc_site_bit(int(seed), L, x, y, z, t, tag))
+
+
+def sites_after(seed, L, xyz, n_half_sweeps):
+    """Spins (+-1) of the sampled sites xyz[n][3] after n_half_sweeps half-sweeps from the
+    T = infinity start of `seed`, each computed from the definition by light-cone recursion."""
+    a = np.ascontiguousarray(xyz, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros(len(a), dtype=np.int8)
+    lib().orc_sites_after(int(seed), int(L), _p(a, C.c_int32), len(a), int(n_half_sweeps),
+                          _p(out, C.c_int8))
+    return out
 
 
 def num_threads() -> int:

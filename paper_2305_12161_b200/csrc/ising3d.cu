@@ -1,0 +1,422 @@
+// libising3d: C ABI (include/ising3d.h) + host launch layer.
+// No CPU fallback anywhere: every compute entry point launches CUDA kernels or fails.
+#include "../../include/ising3d.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "kernels_fused.cuh"
+#include "kernels_generic.cuh"
+#include "kernels_measure.cuh"
+#include "philox.cuh"
+
+namespace {
+
+thread_local std::string g_last_error = "";
+
+int fail(int code, const std::string &msg)
+{
+    g_last_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                     \
+    do {                                                                                   \
+        cudaError_t err__ = (expr);                                                        \
+        if (err__ != cudaSuccess)                                                          \
+            return fail(err__ == cudaErrorMemoryAllocation ? ISING3D_ENOMEM : ISING3D_ECUDA, \
+                        std::string(#expr) + ": " + cudaGetErrorString(err__));            \
+    } while (0)
+
+bool valid_shape(int L, int n_rep) { return L >= 64 && L <= 4096 && (L % 64) == 0 && n_rep >= 1; }
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct ising3d {
+    int L = 0, n_rep = 0;
+    uint64_t sweep = 0;
+    std::vector<uint64_t> seeds;
+    cudaStream_t stream = nullptr;
+    bool owns_mem = false;
+    void *base = nullptr;
+    uint32_t *state[2] = {nullptr, nullptr};   // ping-pong buffers (the fused kernel writes the other one)
+    int cur = 0;
+    uint64_t *d_seeds = nullptr;
+    unsigned long long *d_counts = nullptr;
+    int variant = ISING3D_VARIANT_AUTO;
+    uint64_t launches = 0;
+    int sm_count = 148;
+
+    size_t words_per_replica() const { return (size_t)L * L * L / 32; }
+    size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
+    int counts_per_replica() const { return 1 + 3 * (L / 2 + 1); }
+    bool fused_ok() const { return n_rep == 1 && ising::fused_supported(L); }
+    bool use_fused() const
+    {
+        return variant == ISING3D_VARIANT_FUSED || (variant == ISING3D_VARIANT_AUTO && fused_ok());
+    }
+};
+
+namespace {
+
+struct Layout {
+    size_t state, seeds, counts, total;
+};
+
+Layout make_layout(int L, int n_rep)
+{
+    Layout l;
+    l.state = align_up((size_t)L * L * L / 8 * (size_t)n_rep, 256);
+    l.seeds = align_up((size_t)n_rep * 8, 256);
+    l.counts = align_up((size_t)n_rep * (1 + 3 * (L / 2 + 1)) * 8, 256);
+    l.total = 2 * l.state + l.seeds + l.counts;
+    return l;
+}
+
+int launch_init(ising3d *h)
+{
+    const size_t groups = h->words_per_replica() / 4;
+    dim3 grid((unsigned)((groups + 255) / 256), (unsigned)h->n_rep);
+    ising::init_spins_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds, h->L);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    h->sweep = 0;
+    return ISING3D_OK;
+}
+
+int create(ising3d_t **out, int L, int n_rep, const uint64_t *seeds, void *dev_buf,
+           size_t dev_bytes, void *stream)
+{
+    if (!out || !seeds) return fail(ISING3D_EINVAL, "null pointer");
+    if (!valid_shape(L, n_rep))
+        return fail(ISING3D_EINVAL, "L must be a multiple of 64 in [64, 4096] and n_rep >= 1");
+    if ((size_t)n_rep > 65535) return fail(ISING3D_EINVAL, "n_rep must be <= 65535");
+    const Layout lay = make_layout(L, n_rep);
+    ising3d *h = new (std::nothrow) ising3d();
+    if (!h) return fail(ISING3D_ENOMEM, "host allocation failed");
+    h->L = L;
+    h->n_rep = n_rep;
+    h->seeds.assign(seeds, seeds + n_rep);
+    h->stream = (cudaStream_t)stream;
+    int code = ISING3D_OK;
+    do {
+        cudaError_t e;
+        if (dev_buf) {
+            if (dev_bytes < lay.total || ((uintptr_t)dev_buf & 255)) {
+                code = fail(ISING3D_EINVAL, "device buffer too small or not 256-byte aligned");
+                break;
+            }
+            h->base = dev_buf;
+            h->owns_mem = false;
+        } else {
+            e = cudaMalloc(&h->base, lay.total);
+            if (e != cudaSuccess) {
+                code = fail(e == cudaErrorMemoryAllocation ? ISING3D_ENOMEM : ISING3D_ECUDA,
+                            std::string("cudaMalloc: ") + cudaGetErrorString(e));
+                cudaGetLastError();
+                break;
+            }
+            h->owns_mem = true;
+        }
+        char *p = (char *)h->base;
+        h->state[0] = (uint32_t *)p;
+        h->state[1] = (uint32_t *)(p + lay.state);
+        h->d_seeds = (uint64_t *)(p + 2 * lay.state);
+        h->d_counts = (unsigned long long *)(p + 2 * lay.state + lay.seeds);
+        int dev = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
+            (e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev)) !=
+                cudaSuccess ||
+            (e = cudaMemcpyAsync(h->d_seeds, h->seeds.data(), (size_t)n_rep * 8,
+                                 cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) {
+            code = fail(ISING3D_ECUDA, std::string("setup: ") + cudaGetErrorString(e));
+            break;
+        }
+        // the seeds vector outlives the copy (it lives in the handle)
+        code = launch_init(h);
+    } while (0);
+    if (code != ISING3D_OK) {
+        if (h->owns_mem && h->base) cudaFree(h->base);
+        delete h;
+        return code;
+    }
+    *out = h;
+    return ISING3D_OK;
+}
+
+int sweep_generic(ising3d *h, uint64_t n)
+{
+    const size_t groups = h->words_per_replica() / 8;   // per colour
+    dim3 grid((unsigned)((groups + 255) / 256), (unsigned)h->n_rep);
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint32_t t = (uint32_t)(h->sweep + i);
+        ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
+                                                                     h->L, t, 0);
+        ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
+                                                                     h->L, t, 1);
+    }
+    h->launches += 2 * n;
+    CUDA_TRY(cudaGetLastError());
+    return ISING3D_OK;
+}
+
+int sweep_fused(ising3d *h, uint64_t n)
+{
+    const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint32_t t = (uint32_t)(h->sweep + i);
+        cudaError_t e = ising::launch_fused_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t,
+                                                  keys, h->sm_count, h->stream);
+        if (e != cudaSuccess)
+            return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
+        h->cur = 1 - h->cur;
+        h->launches += 1;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return ISING3D_OK;
+}
+
+// D9: fp64 post-processing of the integer counts, in this exact order.
+void postprocess(int L, uint64_t n_up, const uint64_t *antipar, double c_intercept, double *C,
+                 double *ell)
+{
+    const int nr = L / 2 + 1;
+    const int64_t N = (int64_t)L * L * L;
+    const double m = (double)(2 * (int64_t)n_up - N) / (double)N;
+    std::vector<double> tmp;
+    if (!C) {
+        tmp.resize(nr);
+        C = tmp.data();
+    }
+    for (int r = 0; r < nr; ++r) {
+        const int64_t A = (int64_t)antipar[r] + (int64_t)antipar[nr + r] + (int64_t)antipar[2 * nr + r];
+        const int64_t S = 3 * N - 2 * A;
+        C[r] = (double)S / (double)(3 * N) - m * m;
+    }
+    if (ell) {
+        *ell = std::nan("");
+        for (int r = 0; r + 1 < nr; ++r)
+            if (C[r] >= c_intercept && C[r + 1] < c_intercept) {
+                *ell = (double)r + (C[r] - c_intercept) / (C[r] - C[r + 1]);
+                break;
+            }
+    }
+}
+
+int pow2_floor(int v)
+{
+    int p = 1;
+    while (2 * p <= v) p *= 2;
+    return p;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ising3d_required_bytes(int L, int n_rep)
+{
+    if (!valid_shape(L, n_rep)) return 0;
+    return make_layout(L, n_rep).total;
+}
+
+size_t ising3d_words_per_replica(int L)
+{
+    if (!valid_shape(L, 1)) return 0;
+    return (size_t)L * L * L / 32;
+}
+
+int ising3d_init(ising3d_t **h, int L, uint64_t seed)
+{
+    return create(h, L, 1, &seed, nullptr, 0, nullptr);
+}
+
+int ising3d_init_batch(ising3d_t **h, int L, int n_rep, const uint64_t *seeds)
+{
+    return create(h, L, n_rep, seeds, nullptr, 0, nullptr);
+}
+
+int ising3d_init_batch_with_buffer(ising3d_t **h, int L, int n_rep, const uint64_t *seeds,
+                                   void *dev_buf, size_t dev_bytes, void *cuda_stream)
+{
+    if (!dev_buf) return fail(ISING3D_EINVAL, "null device buffer");
+    return create(h, L, n_rep, seeds, dev_buf, dev_bytes, cuda_stream);
+}
+
+int ising3d_reset(ising3d_t *h)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    return launch_init(h);
+}
+
+int ising3d_set_stream(ising3d_t *h, void *cuda_stream)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->stream = (cudaStream_t)cuda_stream;
+    return ISING3D_OK;
+}
+
+int ising3d_set_variant(ising3d_t *h, int variant)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED)
+        return fail(ISING3D_EINVAL, "unknown variant");
+    if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
+        return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
+    h->variant = variant;
+    return ISING3D_OK;
+}
+
+int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (h->sweep + n_sweeps > 0xFFFFFFFFull || h->sweep + n_sweeps < h->sweep)
+        return fail(ISING3D_EINVAL, "sweep counter would pass 2^32-1");
+    if (n_sweeps == 0) return ISING3D_OK;
+    const int rc = h->use_fused() ? sweep_fused(h, n_sweeps) : sweep_generic(h, n_sweeps);
+    if (rc != ISING3D_OK) return rc;
+    h->sweep += n_sweeps;
+    return ISING3D_OK;
+}
+
+int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
+{
+    if (!h || !out) return fail(ISING3D_EINVAL, "null pointer");
+    if (out->L != h->L || out->n_rep != h->n_rep)
+        return fail(ISING3D_EINVAL, "measurement record shape does not match the handle");
+    if (!out->n_up || !out->n_broken || !out->antipar)
+        return fail(ISING3D_EINVAL, "n_up, n_broken and antipar must be provided");
+    const int L = h->L, WPR = L >> 6, nr = L / 2 + 1, cpr = h->counts_per_replica();
+    const uint32_t *st = h->state[h->cur];
+    CUDA_TRY(cudaMemsetAsync(h->d_counts, 0, (size_t)h->n_rep * cpr * 8, h->stream));
+    {
+        const size_t n4 = h->words_per_replica() / 4;
+        unsigned gx = (unsigned)std::min<size_t>((n4 + 255) / 256, (size_t)h->sm_count * 8);
+        ising::count_up_kernel<<<dim3(gx, h->n_rep), 256, 0, h->stream>>>(
+            st, h->d_counts, h->words_per_replica(), cpr);
+    }
+    {
+        // T[2][L][WX] words of shared memory, WX a power of two
+        int WX = pow2_floor(std::max(1, std::min(WPR, 16384 / L)));
+        const int tiles = (WPR + WX - 1) / WX;
+        const size_t smem = (size_t)2 * L * WX * 4;
+        CUDA_TRY(cudaFuncSetAttribute(ising::measure_yz_kernel<1>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaFuncSetAttribute(ising::measure_yz_kernel<2>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        dim3 grid((unsigned)(L * tiles), (unsigned)h->n_rep);
+        ising::measure_yz_kernel<1><<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, WX, tiles, cpr);
+        ising::measure_yz_kernel<2><<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, WX, tiles, cpr);
+    }
+    {
+        // T[2][RX][WPR]; RX rows per block, RX divides L*L
+        int RX = pow2_floor(std::max(1, 8192 / WPR));
+        while (((size_t)L * L) % RX) RX /= 2;
+        const size_t smem = (size_t)2 * RX * WPR * 4;
+        CUDA_TRY(cudaFuncSetAttribute(ising::measure_x_kernel,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        dim3 grid((unsigned)((size_t)L * L / RX), (unsigned)h->n_rep);
+        ising::measure_x_kernel<<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, RX, cpr);
+    }
+    h->launches += 4;
+    CUDA_TRY(cudaGetLastError());
+    std::vector<unsigned long long> host((size_t)h->n_rep * cpr);
+    CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_counts, host.size() * 8, cudaMemcpyDeviceToHost,
+                             h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    out->sweep = h->sweep;
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        const unsigned long long *c = host.data() + (size_t)rep * cpr;
+        out->n_up[rep] = c[0];
+        uint64_t *a = out->antipar + (size_t)rep * 3 * nr;
+        for (int i = 0; i < 3 * nr; ++i) a[i] = c[1 + i];
+        out->n_broken[rep] = a[1] + a[nr + 1] + a[2 * nr + 1];
+        postprocess(L, out->n_up[rep], a, out->c_intercept,
+                    out->C ? out->C + (size_t)rep * nr : nullptr, out->ell ? out->ell + rep : nullptr);
+    }
+    return ISING3D_OK;
+}
+
+int ising3d_get_state(ising3d_t *h, uint32_t *words, size_t n_words, uint64_t *sweep)
+{
+    if (!h || !words) return fail(ISING3D_EINVAL, "null pointer");
+    if (n_words != h->words_per_replica() * h->n_rep)
+        return fail(ISING3D_EINVAL, "n_words must equal n_rep * L^3/32");
+    CUDA_TRY(cudaMemcpyAsync(words, h->state[h->cur], n_words * 4, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (sweep) *sweep = h->sweep;
+    return ISING3D_OK;
+}
+
+int ising3d_set_state(ising3d_t *h, const uint32_t *words, size_t n_words, uint64_t sweep)
+{
+    if (!h || !words) return fail(ISING3D_EINVAL, "null pointer");
+    if (n_words != h->words_per_replica() * h->n_rep)
+        return fail(ISING3D_EINVAL, "n_words must equal n_rep * L^3/32");
+    if (sweep > 0xFFFFFFFFull) return fail(ISING3D_EINVAL, "sweep counter out of range");
+    CUDA_TRY(cudaMemcpyAsync(h->state[h->cur], words, n_words * 4, cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->sweep = sweep;
+    return ISING3D_OK;
+}
+
+int ising3d_get_state_device(ising3d_t *h, uint32_t *dev_words, size_t n_words, uint64_t *sweep)
+{
+    if (!h || !dev_words) return fail(ISING3D_EINVAL, "null pointer");
+    if (n_words != h->words_per_replica() * h->n_rep)
+        return fail(ISING3D_EINVAL, "n_words must equal n_rep * L^3/32");
+    CUDA_TRY(cudaMemcpyAsync(dev_words, h->state[h->cur], n_words * 4, cudaMemcpyDeviceToDevice,
+                             h->stream));
+    if (sweep) *sweep = h->sweep;
+    return ISING3D_OK;
+}
+
+int ising3d_set_state_device(ising3d_t *h, const uint32_t *dev_words, size_t n_words, uint64_t sweep)
+{
+    if (!h || !dev_words) return fail(ISING3D_EINVAL, "null pointer");
+    if (n_words != h->words_per_replica() * h->n_rep)
+        return fail(ISING3D_EINVAL, "n_words must equal n_rep * L^3/32");
+    if (sweep > 0xFFFFFFFFull) return fail(ISING3D_EINVAL, "sweep counter out of range");
+    CUDA_TRY(cudaMemcpyAsync(h->state[h->cur], dev_words, n_words * 4, cudaMemcpyDeviceToDevice,
+                             h->stream));
+    h->sweep = sweep;
+    return ISING3D_OK;
+}
+
+int ising3d_L(const ising3d_t *h) { return h ? h->L : 0; }
+int ising3d_n_rep(const ising3d_t *h) { return h ? h->n_rep : 0; }
+uint64_t ising3d_sweep_count(const ising3d_t *h) { return h ? h->sweep : 0; }
+uint64_t ising3d_launch_count(const ising3d_t *h) { return h ? h->launches : 0; }
+const char *ising3d_variant_name(const ising3d_t *h)
+{
+    if (!h) return "none";
+    return h->use_fused() ? "fused" : "generic";
+}
+
+int ising3d_sync(ising3d_t *h)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return ISING3D_OK;
+}
+
+void ising3d_free(ising3d_t *h)
+{
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    if (h->owns_mem && h->base) cudaFree(h->base);
+    delete h;
+}
+
+const char *ising3d_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

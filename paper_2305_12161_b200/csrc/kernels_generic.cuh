@@ -1,0 +1,73 @@
+// Generic kernels: any L % 64 == 0, any number of replicas (blockIdx.y = replica).
+//  - init_spins_kernel        a1: T = infinity start from Philox(tag = 1)          (D6)
+//  - halfsweep_generic_kernel a2/a3: one colour, in place, one thread per 128-spin group
+//                              (eq. (6); sweep order PAPER.md:116)
+// Layout D3: state[rep][colour][z][y][wi], wi = 0..L/64-1 32-bit words per row, bit j of
+// word wi = site k = 32 wi + j, x = 2k + ((y+z+colour)&1).
+// Neighbour geometry D4: a colour-c site (k,y,z) has its six neighbours in colour 1-c at
+// (k,y+-1,z), (k,y,z+-1), (k,y,z) and (k-1,y,z) if o = (y+z+c)&1 is 0, else (k+1,y,z).
+#pragma once
+#include "philox.cuh"
+
+namespace ising {
+
+__global__ void __launch_bounds__(256)
+init_spins_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds, int L)
+{
+    const size_t groups_per_colour = (size_t)L * L * (L >> 6) / 4;
+    const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= 2 * groups_per_colour) return;
+    const int rep = blockIdx.y;
+    const uint32_t c = g >= groups_per_colour ? 1u : 0u;
+    const uint32_t q = (uint32_t)(g - c * groups_per_colour);
+    const uint64_t seed = seeds[rep];
+    const uint4 v = philox4x32_10(q, 0u, c, 1u, (uint32_t)seed, (uint32_t)(seed >> 32));
+    reinterpret_cast<uint4 *>(state)[(size_t)rep * 2 * groups_per_colour + g] = v;
+}
+
+__global__ void __launch_bounds__(256)
+halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
+                         int L, uint32_t t, int c)
+{
+    const int WPR = L >> 6;                                   // words per row
+    const size_t WPC = (size_t)L * L * WPR;                   // words per colour
+    const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= WPC / 4) return;
+    const int rep = blockIdx.y;
+    uint32_t *own = state + (size_t)rep * 2 * WPC + (size_t)c * WPC;
+    const uint32_t *oth = state + (size_t)rep * 2 * WPC + (size_t)(1 - c) * WPC;
+    const uint64_t seed = seeds[rep];
+    const uint4 rnd = philox4x32_10((uint32_t)g, t, (uint32_t)c, 0u, (uint32_t)seed,
+                                    (uint32_t)(seed >> 32));
+    const uint32_t rho[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
+    const uint4 sv = reinterpret_cast<const uint4 *>(own)[g];
+    const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+    uint32_t out[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const size_t w = 4 * g + i;
+        const int wi = (int)(w % WPR);
+        const size_t row = w / WPR;
+        const int y = (int)(row % L);
+        const int z = (int)(row / L);
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const uint32_t n_same = oth[w];
+        const uint32_t n_yp = oth[((size_t)z * L + yp) * WPR + wi];
+        const uint32_t n_ym = oth[((size_t)z * L + ym) * WPR + wi];
+        const uint32_t n_zp = oth[((size_t)zp * L + y) * WPR + wi];
+        const uint32_t n_zm = oth[((size_t)zm * L + y) * WPR + wi];
+        uint32_t n_x;
+        if (((y + z + c) & 1) == 0) {       // neighbour at k-1: bit j <- bit j-1
+            const uint32_t prev = oth[row * WPR + (wi == 0 ? WPR - 1 : wi - 1)];
+            n_x = (n_same << 1) | (prev >> 31);
+        } else {                            // neighbour at k+1: bit j <- bit j+1
+            const uint32_t next = oth[row * WPR + (wi == WPR - 1 ? 0 : wi + 1)];
+            n_x = (n_same >> 1) | (next << 31);
+        }
+        out[i] = rule_word(s[i], rho[i], n_same, n_x, n_yp, n_ym, n_zp, n_zm);
+    }
+    reinterpret_cast<uint4 *>(own)[g] = make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+}  // namespace ising

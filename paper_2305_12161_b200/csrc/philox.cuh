@@ -1,0 +1,100 @@
+// Philox4x32-10 for the CUDA path (D5 in DESIGN.md; Salmon et al., SC'11).
+// Counter (c0,c1,c2,c3), key (k0,k1).  One round:
+//   p0 = M0*c0, p1 = M1*c2 (32x32 -> 64 bit);
+//   (c0,c1,c2,c3) <- (hi(p1)^c1^k0, lo(p1), hi(p0)^c3^k1, lo(p0)),
+// ten rounds, the key bumped by (W0,W1) between rounds.
+// Written for the SM: each round is two IMAD.WIDE.U32 (FMA pipe) and two 3-input
+// LOP3 (ALU pipe); the ten round keys are computed once per launch on the host and
+// read from the constant bank (struct PhiloxKeys passed by value), so the key
+// schedule costs no instruction.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ising {
+
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
+constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
+
+struct PhiloxKeys {            // round keys k0 + r*W0, k1 + r*W1, r = 0..9
+    uint32_t k0[10];
+    uint32_t k1[10];
+};
+
+inline PhiloxKeys make_philox_keys(uint64_t seed)
+{
+    PhiloxKeys k;
+    uint32_t a = (uint32_t)(seed & 0xFFFFFFFFull), b = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        k.k0[r] = a;
+        k.k1[r] = b;
+        a += kPhiloxW0;
+        b += kPhiloxW1;
+    }
+    return k;
+}
+
+// round keys from the constant bank (single lattice)
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKeys &k)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// key schedule in registers (batched replicas: the seed is per block)
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += kPhiloxW0;
+        k1 += kPhiloxW1;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// ---------------------------------------------------------------------------
+// The site rule on 32 sites at once (eq. (6), D2).
+// n1..n6: the six neighbour words (bit = 1 <=> spin up), s: own word, rho: tie bits.
+// With U = number of up neighbours the rule is  new = [U + (s ^ rho) >= 4]:
+//   U >= 4 -> up, U <= 2 -> down (Delta E < 0 flips, > 0 keeps), U = 3 (Delta E = 0)
+//   -> s ^ rho, i.e. flip iff the random bit is 1.
+// Seven one-bit inputs, threshold 4: two 3:2 compressors, then two majorities.
+// 7 LOP3 per word.
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c)
+{
+    return (a & b) | (c & (a | b));
+}
+
+__device__ __forceinline__ uint32_t rule_word(uint32_t s, uint32_t rho, uint32_t n1, uint32_t n2,
+                                              uint32_t n3, uint32_t n4, uint32_t n5, uint32_t n6)
+{
+    const uint32_t sa = n1 ^ n2 ^ n3, ca = maj3(n1, n2, n3);
+    const uint32_t sb = n4 ^ n5 ^ n6, cb = maj3(n4, n5, n6);
+    const uint32_t m = maj3(sa, sb, s ^ rho);
+    return maj3(ca, cb, m);
+}
+
+}  // namespace ising

@@ -1,0 +1,321 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bit-exact for the packed state and all integer counts; C(r) and
+ell within 1e-12 relative (BASELINE.json north_star)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2305_12161_b200 import inputs  # noqa: E402
+
+RTOL = 1e-12     # north_star: "ell(t) and the normalised C(r,t) ... within 1e-12 relative"
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2305_12161_b200 import build, binding
+    build.build()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    oracle.build()
+    return oracle
+
+
+def check_measure(got, want, rep=0):
+    assert int(got["n_up"][rep]) == want["n_up"]
+    assert np.array_equal(got["antipar"][rep], want["antipar"])
+    assert int(got["n_broken"][rep]) == want["n_broken"]
+    assert got["sweep"] == want["sweep"]
+    C_got, C_want = got["C"][rep], want["C"]
+    assert np.all(np.abs(C_got - C_want) <= RTOL * np.abs(C_want))
+    if math.isnan(want["ell"]):
+        assert math.isnan(got["ell"][rep])
+    else:
+        assert abs(got["ell"][rep] - want["ell"]) <= RTOL * abs(want["ell"])
+
+
+def run_against_oracle(B, orc, L, seed, checkpoints, variant, measure_at=None, thin_r=None):
+    sim = B.Ising3D(L, [seed], variant=variant)
+    ref = orc.Oracle(L, seed)
+    assert np.array_equal(sim.get_state(), ref.export_words()), "T=inf start differs"
+    t = 0
+    for cp in checkpoints:
+        sim.sweep(cp - t)
+        ref.sweep(cp - t)
+        t = cp
+        assert sim.sweep_count == cp == ref.sweep_count
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+        if measure_at is None or cp in measure_at:
+            got = sim.measure()
+            if thin_r is None:
+                check_measure(got, ref.measure_full())
+            else:
+                n_up, a = ref.measure(thin_r)
+                assert int(got["n_up"][0]) == n_up
+                assert np.array_equal(got["antipar"][0][:, thin_r], a)
+    sim.free()
+    return ref
+
+
+# ------------------------------------------------------------------ config 1
+def test_config1_L64_all_checkpoints(B, orc):
+    w = inputs.WORKLOADS["config1_L64"]
+    run_against_oracle(B, orc, w["L"], w["seeds"][0], w["times"], B.VARIANT_AUTO)
+
+
+@pytest.mark.parametrize("L,seed,cps", [(128, 7, [1, 2, 5, 12]), (192, 8, [1, 3, 6]), (320, 9, [1, 2])])
+def test_generic_kernel_other_sizes(B, orc, L, seed, cps):
+    """Rows of 2, 3 and 5 words: ragged measurement tiles, non-power-of-two rows."""
+    run_against_oracle(B, orc, L, seed, cps, B.VARIANT_GENERIC)
+
+
+# ------------------------------------------------------------------ config 2
+def test_config2_L256_fused_prefix(B, orc):
+    run_against_oracle(B, orc, 256, 2, inputs.measurement_times(60), B.VARIANT_FUSED,
+                       measure_at={1, 10, 60})
+
+
+def test_config2_L256_generic_prefix(B, orc):
+    run_against_oracle(B, orc, 256, 2, [1, 2, 3, 10, 25], B.VARIANT_GENERIC, measure_at={25})
+
+
+@pytest.mark.slow
+def test_config2_L256_full_run(B, orc):
+    """All 2000 sweeps of config 2, state compared at all 23 log-spaced checkpoints."""
+    w = inputs.WORKLOADS["config2_L256"]
+    if os.environ.get("ISING3D_SHORT_TESTS"):
+        pytest.skip("short test mode")
+    run_against_oracle(B, orc, 256, w["seeds"][0], w["times"], B.VARIANT_AUTO,
+                       measure_at={100, 2000})
+
+
+# ------------------------------------------------------------------ fused kernel, larger rows
+@pytest.mark.parametrize("L,seed,cps", [(512, 11, [1, 2, 4]), (1024, 3, [1, 2])])
+def test_fused_kernel_larger_L(B, orc, L, seed, cps):
+    thin = None if L <= 512 else np.array([0, 1, 2, 3, 7, 64, 255, 256, 511, 512], dtype=np.int32)
+    run_against_oracle(B, orc, L, seed, cps, B.VARIANT_FUSED, measure_at={cps[-1]}, thin_r=thin)
+
+
+@pytest.mark.parametrize("L", [256, 512, 1024, 2048])
+def test_fused_equals_generic(B, L):
+    """Not an oracle check: the two kernels must agree bit for bit (also at sizes and times
+    the oracle cannot reach); the generic kernel is oracle-checked above."""
+    a = B.Ising3D(L, [5], variant=B.VARIANT_FUSED)
+    b = B.Ising3D(L, [5], variant=B.VARIANT_GENERIC)
+    assert a.variant_name == "fused" and b.variant_name == "generic"
+    for n in (1, 2, 7):
+        a.sweep(n)
+        b.sweep(n)
+        assert np.array_equal(a.get_state(), b.get_state())
+    a.free()
+    b.free()
+
+
+# ------------------------------------------------------------------ config 5 (full size, sampled)
+def _sample_sites(L, n, seed, RPT=28):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    xyz = rng.integers(0, L, size=(n, 3))
+    # force the structural edges: row ends / word and group boundaries in x, y-tile borders of
+    # the fused kernel (multiples of RPT and the wrap), z-chunk borders and the z wrap
+    xs = [0, 1, 2, 63, 64, 65, 255, 256, 257, L // 2 - 1, L // 2, L - 2, L - 1]
+    ys = [0, 1, 2, RPT - 2, RPT - 1, RPT, RPT + 1, 2 * RPT - 1, 2 * RPT, L - 3, L - 2, L - 1]
+    zs = [0, 1, 2, 3, L // 6, L // 6 + 1, L // 3, L // 3 + 1, L // 2, L - 3, L - 2, L - 1]
+    k = 0
+    for x in xs:
+        for y in ys[::2]:
+            for z in zs[::3]:
+                xyz[k] = (x, y, z)
+                k += 1
+    for y in ys:
+        for z in zs:
+            xyz[k] = (int(rng.integers(0, L)), y, z)
+            k += 1
+    assert k < n
+    return xyz.astype(np.int32)
+
+
+def _bits_at(words, L, xyz):
+    wpc = L ** 3 // 64
+    x, y, z = xyz[:, 0].astype(np.int64), xyz[:, 1].astype(np.int64), xyz[:, 2].astype(np.int64)
+    c = (x + y + z) & 1
+    b = (z * L + y) * (L // 2) + (x >> 1)
+    w = words[c * wpc + (b >> 5)]
+    return np.where((w >> (b & 31).astype(np.uint32)) & 1, 1, -1).astype(np.int8)
+
+
+@pytest.mark.parametrize("L,seed,variant", [(2048, 4, "fused"), (2048, 4, "generic"), (1024, 3, "fused")])
+def test_full_size_sampled_sites(B, orc, L, seed, variant):
+    """Config 5 / 4 at full size in the launch configuration bench.py times: sampled sites
+    after 0, 1 and 2 sweeps against values the oracle computes one by one from the
+    definition (light-cone recursion, no GPU data involved)."""
+    sim = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC)
+    xyz = _sample_sites(L, 3000, 17)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    for n_sweeps in (0, 1, 2):
+        if n_sweeps:
+            sim.sweep(1)
+        got = _bits_at(sim.get_state(buf), L, xyz)
+        want = orc.sites_after(seed, L, xyz, 2 * n_sweeps)
+        bad = np.nonzero(got != want)[0]
+        assert bad.size == 0, "sweep %d: %d sampled sites differ, first %s" % (
+            n_sweeps, bad.size, xyz[bad[:5]].tolist())
+    # properties that hold at any size
+    m = sim.measure()
+    N = L ** 3
+    assert int(m["n_broken"][0]) == int(m["antipar"][0][:, 1].sum())
+    assert np.all(m["antipar"][0][:, 0] == 0)
+    assert 0 < int(m["n_up"][0]) < N
+    e_prev = int(m["n_broken"][0])
+    sim.sweep(1)
+    m2 = sim.measure()
+    assert int(m2["n_broken"][0]) <= e_prev          # energy never increases at T = 0
+    sim.free()
+
+
+def test_L2048_measurement_closed_form(B):
+    """Measurement kernels at full size on the slab state (closed form pinned in the oracle
+    tests): A_axis(r) = 2 r L^2, others 0, m = 0, ell = 3L/8."""
+    L = 2048
+    sim = B.Ising3D(L, [1])
+    wpc = L ** 3 // 64
+    words = np.zeros(2 * wpc, dtype=np.uint32)
+    # slab of +1 for z in [100, 100 + L/2): whole planes of both colours
+    per_plane = L * (L // 64)
+    for c in (0, 1):
+        words[c * wpc + 100 * per_plane: c * wpc + (100 + L // 2) * per_plane] = 0xFFFFFFFF
+    sim.set_state(words, 0)
+    m = sim.measure()
+    r = np.arange(L // 2 + 1, dtype=np.uint64)
+    assert int(m["n_up"][0]) == L ** 3 // 2
+    assert np.array_equal(m["antipar"][0][2], 2 * r * L * L)
+    assert not m["antipar"][0][0].any() and not m["antipar"][0][1].any()
+    assert abs(m["ell"][0] - 3 * L / 8) <= 1e-9
+    sim.sweep(2)                                     # flat interfaces are fixed points
+    assert np.array_equal(sim.get_state(), words)
+    sim.free()
+
+
+# ------------------------------------------------------------------ config 3 (batch)
+def test_config3_batch_equals_singles_and_oracle(B, orc):
+    L = 128
+    seeds = inputs.WORKLOADS["config3_64xL128"]["seeds"]
+    batch = B.Ising3D(L, seeds)
+    assert batch.n_rep == 64
+    wpr = L ** 3 // 32
+    cps = [1, 2, 5, 20]
+    refs = {s: orc.Oracle(L, s) for s in (100, 101, 131, 163)}
+    singles = {s: B.Ising3D(L, [s]) for s in (100, 117, 163)}
+    t = 0
+    for cp in cps:
+        batch.sweep(cp - t)
+        st = batch.get_state().reshape(64, wpr)
+        meas = batch.measure()
+        for s, ref in refs.items():
+            ref.sweep(cp - t)
+            assert np.array_equal(st[s - 100], ref.export_words())
+            check_measure(meas, ref.measure_full(), rep=s - 100)
+        for s, one in singles.items():
+            one.sweep(cp - t)
+            assert np.array_equal(st[s - 100], one.get_state())
+        t = cp
+    # distinct seeds give distinct lattices
+    assert not np.array_equal(st[0], st[1])
+    batch.free()
+    for one in singles.values():
+        one.free()
+
+
+# ------------------------------------------------------------------ set_state / structured inputs
+@pytest.mark.parametrize("L,variant", [(64, "generic"), (128, "generic"), (256, "fused"), (256, "generic")])
+def test_set_state_random_and_coarse_inputs(B, orc, L, variant):
+    v = B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC
+    for words, t0 in [(inputs.random_words(L, 1, 123), 0), (inputs.coarse_words(L, 5), 1000),
+                      (inputs.coarse_words(L, 6, block=16), 4_000_000_000)]:
+        sim = B.Ising3D(L, [77], variant=v)
+        sim.set_state(words, t0)
+        ref = orc.Oracle(L, 77, init=False)
+        ref.import_words(words, t0)
+        assert np.array_equal(sim.get_state(), words)
+        for n in (1, 3):
+            sim.sweep(n)
+            ref.sweep(n)
+            assert np.array_equal(sim.get_state(), ref.export_words())
+        check_measure(sim.measure(), ref.measure_full())
+        sim.free()
+
+
+@pytest.mark.parametrize("variant", ["generic", "fused"])
+def test_structured_states(B, orc, variant):
+    """Fixed points, Neel state, single spins and 2x2x2 cubes across every periodic wrap."""
+    L = 256 if variant == "fused" else 64
+    v = B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC
+    states = [inputs.all_up(L), -inputs.all_up(L), inputs.neel(L), -inputs.neel(L)]
+    for axis in (0, 1, 2):
+        states.append(inputs.slab(L, axis, L - 1, 2))
+        states.append(inputs.slab(L, axis, 5, L // 2))
+    for pos in [(0, 0, 0), (L - 1, L - 1, L - 1), (L - 1, 0, 3), (63, 31, L - 1), (64, 0, 0)]:
+        states.append(inputs.single_spin(L, *pos))
+        states.append(inputs.cube(L, *pos))
+    sim = B.Ising3D(L, [2024], variant=v)
+    for s0 in states:
+        words = inputs.pack_spins(s0)
+        ref = orc.Oracle(L, 2024, init=False)
+        for t0 in (0, 17):
+            sim.set_state(words, t0)
+            ref.import_words(words, t0)
+            sim.sweep(2)
+            ref.sweep(2)
+            assert np.array_equal(sim.get_state(), ref.export_words())
+        check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+
+
+def test_checkpoint_resume_and_reset(B, orc):
+    L = 256
+    a = B.Ising3D(L, [31])
+    a.sweep(9)
+    b = B.Ising3D(L, [31])
+    b.sweep(4)
+    w = b.get_state()
+    c = B.Ising3D(L, [999])          # the seed is part of the state: same seed needed
+    c.free()
+    c = B.Ising3D(L, [31])
+    c.set_state(w, 4)
+    c.sweep(5)
+    assert np.array_equal(a.get_state(), c.get_state()) and c.sweep_count == 9
+    first = B.Ising3D(L, [31]).get_state()
+    a.reset()
+    assert a.sweep_count == 0 and np.array_equal(a.get_state(), first)
+    ref = orc.Oracle(L, 31)
+    assert np.array_equal(first, ref.export_words())
+    for s in (a, b, c):
+        s.free()
+
+
+def test_library_owned_memory_and_errors(B, orc):
+    sim = B.Ising3D(64, [1], torch_buffer=False)
+    ref = orc.Oracle(64, 1)
+    sim.sweep(2)
+    ref.sweep(2)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    with pytest.raises(B.Ising3DError):
+        sim.set_variant(B.VARIANT_FUSED)            # L = 64 has no fused kernel
+    with pytest.raises(B.Ising3DError):
+        sim.set_state(np.zeros(5, dtype=np.uint32), 0)
+    sim.set_state(ref.export_words(), 2 ** 32 - 2)
+    sim.sweep(1)
+    with pytest.raises(B.Ising3DError):
+        sim.sweep(1)                                # counter would pass 2^32 - 1
+    assert sim.launch_count > 0
+    sim.free()
+    with pytest.raises(B.Ising3DError):
+        B.Ising3D(100, [1])

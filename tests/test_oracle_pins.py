@@ -503,3 +503,19 @@ def test_threads_do_not_change_results():
     rb = b.measure_full()
     assert np.array_equal(a.spins, b.spins)
     assert ra["n_up"] == rb["n_up"] and np.array_equal(ra["antipar"], rb["antipar"])
+
+
+def test_site_after_equals_full_lattice():
+    """The one-site light-cone recursion (used for sampled parity at L = 2048) against the
+    array version, every site, L = 6 and 8, up to 2 sweeps."""
+    for L, seed in [(6, 13), (8, 14)]:
+        z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+        xyz = np.stack([x.ravel(), y.ravel(), z.ravel()], axis=1)
+        o = orc.Oracle(L, seed)
+        assert np.array_equal(orc.sites_after(seed, L, xyz, 0), o.spins.ravel())
+        h = 0
+        for t in range(2):
+            for c in (0, 1):
+                o.half_sweep(t, c)
+                h += 1
+                assert np.array_equal(orc.sites_after(seed, L, xyz, h), o.spins.ravel())
