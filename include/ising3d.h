@@ -75,6 +75,7 @@ extern "C" {
 #define ISING3D_VARIANT_AUTO    0   /* fused kernel where the shape allows, else generic */
 #define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
 #define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
+#define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096)        */
 
 typedef struct ising3d ising3d_t;   /* opaque */
 

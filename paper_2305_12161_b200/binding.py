@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libising3d.so")
 
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
-VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED = 0, 1, 2
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2 = 0, 1, 2, 3
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",

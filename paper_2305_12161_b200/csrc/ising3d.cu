@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "kernels_fused.cuh"
+#include "kernels_fused2.cuh"
 #include "kernels_generic.cuh"
 #include "kernels_measure.cuh"
 #include "philox.cuh"
@@ -59,9 +60,15 @@ struct ising3d {
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
     int counts_per_replica() const { return 1 + 3 * (L / 2 + 1); }
     bool fused_ok() const { return n_rep == 1 && ising::fused_supported(L); }
+    bool fused2_ok() const { return n_rep == 1 && ising::fused2_supported(L); }
+    bool use_fused2() const
+    {
+        return variant == ISING3D_VARIANT_FUSED2 || (variant == ISING3D_VARIANT_AUTO && fused2_ok());
+    }
     bool use_fused() const
     {
-        return variant == ISING3D_VARIANT_FUSED || (variant == ISING3D_VARIANT_AUTO && fused_ok());
+        return variant == ISING3D_VARIANT_FUSED ||
+               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok());
     }
 };
 
@@ -168,13 +175,16 @@ int sweep_generic(ising3d *h, uint64_t n)
     return ISING3D_OK;
 }
 
-int sweep_fused(ising3d *h, uint64_t n)
+int sweep_fused(ising3d *h, uint64_t n, bool gen2)
 {
     const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
     for (uint64_t i = 0; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
-        cudaError_t e = ising::launch_fused_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t,
-                                                  keys, h->sm_count, h->stream);
+        cudaError_t e =
+            gen2 ? ising::launch_fused2_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t,
+                                              h->seeds[0], h->sm_count, h->stream)
+                 : ising::launch_fused_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t, keys,
+                                             h->sm_count, h->stream);
         if (e != cudaSuccess)
             return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
         h->cur = 1 - h->cur;
@@ -268,10 +278,12 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream)
 int ising3d_set_variant(ising3d_t *h, int variant)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED)
+    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED2)
         return fail(ISING3D_EINVAL, "unknown variant");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
         return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
+    if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())
+        return fail(ISING3D_EINVAL, "fused2 kernel needs n_rep == 1 and L in {512,1024,2048,4096}");
     h->variant = variant;
     return ISING3D_OK;
 }
@@ -282,7 +294,9 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xFFFFFFFFull || h->sweep + n_sweeps < h->sweep)
         return fail(ISING3D_EINVAL, "sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return ISING3D_OK;
-    const int rc = h->use_fused() ? sweep_fused(h, n_sweeps) : sweep_generic(h, n_sweeps);
+    const int rc = h->use_fused2()  ? sweep_fused(h, n_sweeps, true)
+                   : h->use_fused() ? sweep_fused(h, n_sweeps, false)
+                                    : sweep_generic(h, n_sweeps);
     if (rc != ISING3D_OK) return rc;
     h->sweep += n_sweeps;
     return ISING3D_OK;
@@ -399,7 +413,7 @@ uint64_t ising3d_launch_count(const ising3d_t *h) { return h ? h->launches : 0; 
 const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";
-    return h->use_fused() ? "fused" : "generic";
+    return h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
 }
 
 int ising3d_sync(ising3d_t *h)

@@ -1,0 +1,366 @@
+// Fused full-sweep kernel, second generation (a2+a3+a4 in one launch), L in {512..4096}.
+//
+// Same data flow as kernels_fused.cuh (z-march, bulk-async plane tiles in a shared-memory
+// ring, black at plane z then white at plane z-1 on the updated black spins, ping-pong
+// src -> dst), re-organised around what the first ncu capture showed (instruction-bound:
+// ALU pipe 54 %, issue 58 %, 310 warp instructions per group pair against ~185 needed):
+//
+//  * every thread owns TWO adjacent rows (even tile row 2p and odd row 2p+1) of one 128-spin
+//    group column.  The in-row neighbour direction o = (y+z+c)&1 (D4) is then the same for
+//    all threads of the CTA at a given step (even row: o = z&1, odd row: the opposite), so
+//    the one-bit funnel shifts are compile-time left/right, and one of the two y-neighbours
+//    of each row is already in the thread's registers (half the shared-memory reads).
+//  * the march is unrolled 6 planes deep (lcm of the 3-slot register windows and the
+//    2-periodic shift direction): the windows W_old[z-1..z+1], B_new[z-2..z] rotate by
+//    renaming, not by moves.
+//  * tiles are 2*NT/R4 rows tall (64 rows at L = 2048) with the same 2+2 halo rows, so the
+//    recomputed fraction halves.
+//  * Philox4x32-10: everything that depends only on (t, colour, key) is folded on the host
+//    per launch (round 0 has one variable product, round 1 one), the rest reads its round
+//    keys from the constant bank: 18 IMAD.WIDE + 19 LOP3 per 128 sites.
+//
+// Site rule: eq. (6) PAPER.md:105-108 (D2); sweep order PAPER.md:116 (D7); random bits D5.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "kernels_fused.cuh"   // mbarrier / bulk-copy helpers, rule_group
+#include "philox.cuh"
+
+namespace ising {
+
+constexpr int kF2Stages = 4;     // shared-memory ring depth S; prefetch distance S-1
+
+// Per-launch Philox constants (host-folded, D5): counter (q, t, colour, 0), key (k0, k1).
+struct SweepConsts {
+    uint32_t a0;        // round-0 output c0 = t ^ k0[0]           (hi(M1*colour) = 0)
+    uint32_t r0k1;      // k1[0]:        round-0 c2 = hi(M0*q) ^ k1[0]
+    uint32_t c1[2];     // (M1*colour) ^ k0[1]: round-1 c0 = hi(M1*c2) ^ c1[colour]
+    uint32_t d1;        // hi(M0*a0) ^ k1[1]:   round-1 c2 = lo(M0*q) ^ d1
+    uint32_t e2;        // lo(M0*a0) ^ k1[2]:   round-2 c2 = hi(M0*c0) ^ e2
+    uint32_t k0[10];    // round keys
+    uint32_t k1[10];
+};
+
+inline SweepConsts make_sweep_consts(uint64_t seed, uint32_t t)
+{
+    SweepConsts s;
+    const PhiloxKeys k = make_philox_keys(seed);
+    for (int r = 0; r < 10; ++r) {
+        s.k0[r] = k.k0[r];
+        s.k1[r] = k.k1[r];
+    }
+    s.a0 = t ^ k.k0[0];
+    s.r0k1 = k.k1[0];
+    s.c1[0] = 0u ^ k.k0[1];
+    s.c1[1] = kPhiloxM1 ^ k.k0[1];
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * s.a0;
+    s.d1 = (uint32_t)(p0 >> 32) ^ k.k1[1];
+    s.e2 = (uint32_t)p0 ^ k.k1[2];
+    return s;
+}
+
+// Philox4x32-10 of counter (q, t, COL, 0) with the constants above; bit-identical to
+// philox4x32_10(q, t, COL, 0, keys) (checked against the oracle by the parity tests).
+template <int COL>
+__device__ __forceinline__ uint4 philox_folded(const uint32_t q, const SweepConsts &k)
+{
+    // round 0: p0 = M0*q, p1 = M1*COL (constant, hi = 0)
+    const uint64_t q0 = (uint64_t)kPhiloxM0 * q;
+    uint32_t c2 = (uint32_t)(q0 >> 32) ^ k.r0k1;
+    // round 1: p0 = M0*a0 (constant), p1 = M1*c2
+    const uint64_t p1a = (uint64_t)kPhiloxM1 * c2;
+    uint32_t c0 = (uint32_t)(p1a >> 32) ^ k.c1[COL];
+    uint32_t c1 = (uint32_t)p1a;
+    c2 = (uint32_t)q0 ^ k.d1;
+    // round 2: c3 = lo(M0*a0) folded into e2
+    uint32_t c3;
+    {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.k0[2];
+        c2 = (uint32_t)(p0 >> 32) ^ k.e2;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+    }
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k.k0[r];
+        c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// x-neighbour word with a compile-time direction (D4): O = 0 -> neighbour k-1, edge = word 3
+// of the previous group of the row; O = 1 -> neighbour k+1, edge = word 0 of the next group.
+template <int O>
+__device__ __forceinline__ uint4 xshift_t(const uint4 w, const uint32_t edge)
+{
+    uint4 r;
+    if (O == 0) {
+        r.x = __funnelshift_l(edge, w.x, 1);
+        r.y = __funnelshift_l(w.x, w.y, 1);
+        r.z = __funnelshift_l(w.y, w.z, 1);
+        r.w = __funnelshift_l(w.z, w.w, 1);
+    } else {
+        r.x = __funnelshift_r(w.x, w.y, 1);
+        r.y = __funnelshift_r(w.y, w.z, 1);
+        r.z = __funnelshift_r(w.z, w.w, 1);
+        r.w = __funnelshift_r(w.w, edge, 1);
+    }
+    return r;
+}
+
+template <int O>
+__device__ __forceinline__ uint4 xneigh(const uint4 w, const int lane_prev, const int lane_next)
+{
+    const uint32_t edge = __shfl_sync(0xffffffffu, O ? w.x : w.w, O ? lane_next : lane_prev);
+    return xshift_t<O>(w, edge);
+}
+
+// Register windows of one thread: [slot][row]; the slot <-> plane assignment rotates with the
+// step phase PH = k mod 3 (W: slot PH = z-1, PH+1 = z, PH+2 = z+1; B_new: PH = z-2, PH+1 = z-1,
+// PH+2 = z), all indices compile-time after unrolling.
+struct F2Win {
+    uint4 W[3][2];
+    uint4 B[3][2];
+};
+
+struct F2Ctx {
+    const uint4 *Wst, *Bst;     // shared-memory ring [S][PLANE]
+    uint4 *nb;                  // [2][PLANE] B_new planes for the y+-1 exchange
+    uint64_t *bars;
+    uint4 *dstB, *dstW;         // colour bases of the destination state
+    int si0, si_ym, si_yp;      // own position (row 2p) / row 2p-1 / row 2p+2 in a plane tile
+    int lane_prev, lane_next;
+    uint32_t qrow, qplane;      // Philox group index of (row 2p, x4) inside a plane; groups/plane
+    bool ok0, ok1;              // rows whose results this CTA stores
+    int nz;
+};
+
+template <int R4, int PLANE, int PH, int O>
+__device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const int z,
+                                        const SweepConsts &keys)
+{
+    constexpr int S = kF2Stages;
+    constexpr int M = PH % 3, Z = (PH + 1) % 3, P = (PH + 2) % 3;
+    const int s = k & (S - 1);
+    mbar_wait(smem_u32(&c.bars[s]), (uint32_t)((k / S) & 1));
+    const uint4 *Wnew = c.Wst + s * PLANE;
+    const uint4 *Bold = c.Bst + s * PLANE;
+    const uint4 *Wz = c.Wst + ((k - 1) & (S - 1)) * PLANE;       // plane z of W_old
+    w.W[P][0] = Wnew[c.si0];
+    w.W[P][1] = Wnew[c.si0 + R4];
+    const uint4 Bo0 = Bold[c.si0], Bo1 = Bold[c.si0 + R4];
+    // ---- black update at plane z (colour 0); even row: o = O, odd row: o = 1-O ----
+    {
+        const uint4 Wym = Wz[c.si_ym], Wyp = Wz[c.si_yp];
+        const uint32_t q = (uint32_t)z * c.qplane + c.qrow;
+        const uint4 rho0 = philox_folded<0>(q, keys);
+        const uint4 rho1 = philox_folded<0>(q + R4, keys);
+        const uint4 Wx0 = xneigh<O>(w.W[Z][0], c.lane_prev, c.lane_next);
+        const uint4 Wx1 = xneigh<1 - O>(w.W[Z][1], c.lane_prev, c.lane_next);
+        w.B[P][0] = rule_group(Bo0, rho0, w.W[Z][0], Wx0, Wym, w.W[Z][1], w.W[M][0], w.W[P][0]);
+        w.B[P][1] = rule_group(Bo1, rho1, w.W[Z][1], Wx1, w.W[Z][0], Wyp, w.W[M][1], w.W[P][1]);
+        uint4 *nbw = c.nb + (k & 1) * PLANE + c.si0;
+        nbw[0] = w.B[P][0];
+        nbw[R4] = w.B[P][1];
+        if (k >= 3 && k < 3 + c.nz) {
+            uint4 *d = c.dstB + (size_t)((uint32_t)z * c.qplane + c.qrow);
+            if (c.ok0) d[0] = w.B[P][0];
+            if (c.ok1) d[R4] = w.B[P][1];
+        }
+    }
+    // ---- white update at plane z-1 (colour 1) on the updated black spins ----
+    {
+        const uint4 *Bz = c.nb + ((k - 1) & 1) * PLANE;          // B_new[z-1], written last step
+        const uint4 Bym = Bz[c.si_ym], Byp = Bz[c.si_yp];
+        const int zw = z == 0 ? (int)(c.qplane / R4) - 1 : z - 1;
+        const uint32_t q = (uint32_t)zw * c.qplane + c.qrow;
+        const uint4 rho0 = philox_folded<1>(q, keys);
+        const uint4 rho1 = philox_folded<1>(q + R4, keys);
+        const uint4 Bx0 = xneigh<O>(w.B[Z][0], c.lane_prev, c.lane_next);
+        const uint4 Bx1 = xneigh<1 - O>(w.B[Z][1], c.lane_prev, c.lane_next);
+        const uint4 nW0 =
+            rule_group(w.W[M][0], rho0, w.B[Z][0], Bx0, Bym, w.B[Z][1], w.B[M][0], w.B[P][0]);
+        const uint4 nW1 =
+            rule_group(w.W[M][1], rho1, w.B[Z][1], Bx1, w.B[Z][0], Byp, w.B[M][1], w.B[P][1]);
+        if (k >= 4) {
+            uint4 *d = c.dstW + (size_t)q;
+            if (c.ok0) d[0] = nW0;
+            if (c.ok1) d[R4] = nW1;
+        }
+    }
+}
+
+// Grid: blockIdx.x = y tile (RPT stored rows each, RPT even), blockIdx.y = z chunk.
+// Chunk boundaries are odd planes, so the first marched plane z0 = zs-3 is even and the
+// in-row direction of the even tile row at step k is k & 1.
+template <int R4, int NT>
+__global__ void __launch_bounds__(NT, 2)
+fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, const int L,
+                    const int RPT, const int nzc, const __grid_constant__ SweepConsts keys)
+{
+    constexpr int TY = 2 * NT / R4;    // rows in the tile (incl. 2+2 halo rows)
+    constexpr int PLANE = TY * R4;     // uint4 per plane tile
+    constexpr int S = kF2Stages, D = S - 1;
+    static_assert(R4 <= 32 && (32 % R4) == 0, "a row must fit a warp");
+
+    extern __shared__ __align__(128) uint4 smem[];
+    uint4 *Wst = smem;                     // [S][PLANE]  W_old planes
+    uint4 *Bst = smem + S * PLANE;         // [S][PLANE]  B_old planes
+    uint4 *nb = smem + 2 * S * PLANE;      // [2][PLANE]  B_new planes (y+-1 exchange)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(nb + 2 * PLANE);
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int x4 = tid & (R4 - 1), p = tid / R4;     // group column, row pair
+    const int ry = 2 * p;                            // even tile row of this thread
+    const int jt = blockIdx.x, zc = blockIdx.y;
+    const int zs = ((int)((long long)L * zc / nzc)) | 1;
+    const int ze = zc + 1 == nzc ? (L | 1) : (((int)((long long)L * (zc + 1) / nzc)) | 1);
+    const int nz = ze - zs;
+    const int K = nz + 4;                  // steps: 2 window fills, nz+1 black, nz white
+    int ybase = jt * RPT - 2;
+    if (ybase < 0) ybase += L;
+    int y = ybase + ry;
+    if (y >= L) y -= L;
+    const size_t G = (size_t)L * L * R4;   // groups per colour
+
+    F2Ctx c;
+    c.Wst = Wst;
+    c.Bst = Bst;
+    c.nb = nb;
+    c.bars = bars;
+    c.dstB = dst;
+    c.dstW = dst + G;
+    c.si0 = ry * R4 + x4;
+    c.si_ym = ry > 0 ? c.si0 - R4 : c.si0;
+    c.si_yp = ry + 2 < TY ? c.si0 + 2 * R4 : c.si0;
+    c.lane_prev = (lane & ~(R4 - 1)) | ((lane - 1) & (R4 - 1));
+    c.lane_next = (lane & ~(R4 - 1)) | ((lane + 1) & (R4 - 1));
+    c.qrow = (uint32_t)(y * R4 + x4);
+    c.qplane = (uint32_t)(L * R4);
+    c.ok0 = (ry >= 2) && (ry - 2 < RPT) && (jt * RPT + ry - 2 < L);
+    c.ok1 = (ry + 1 - 2 < RPT) && (ry + 1 < TY - 2) && (jt * RPT + ry + 1 - 2 < L) && (ry >= 2);
+    c.nz = nz;
+
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) mbar_init(smem_u32(&bars[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // producer: stage k holds W_old[z0+1+k] and B_old[z0+k], z0 = zs-3 (periodic)
+    const int n1 = min(TY, L - ybase);     // rows before the periodic wrap in y
+    auto issue = [&](int k) {
+        const int s = k & (S - 1);
+        int zw = zs - 2 + k;
+        zw = (zw % L + L) % L;
+        int zb = zs - 3 + k;
+        zb = (zb % L + L) % L;
+        const uint32_t bar = smem_u32(&bars[s]);
+        const uint32_t bytes = (uint32_t)PLANE * 16u;
+        mbar_expect_tx(bar, 2 * bytes);
+        const uint4 *gw = src + G + ((size_t)zw * L) * R4;
+        const uint4 *gb = src + ((size_t)zb * L) * R4;
+        bulk_g2s(smem_u32(Wst + s * PLANE), gw + (size_t)ybase * R4, (uint32_t)n1 * R4 * 16u, bar);
+        bulk_g2s(smem_u32(Bst + s * PLANE), gb + (size_t)ybase * R4, (uint32_t)n1 * R4 * 16u, bar);
+        if (n1 < TY) {
+            bulk_g2s(smem_u32(Wst + s * PLANE + n1 * R4), gw, (uint32_t)(TY - n1) * R4 * 16u, bar);
+            bulk_g2s(smem_u32(Bst + s * PLANE + n1 * R4), gb, (uint32_t)(TY - n1) * R4 * 16u, bar);
+        }
+    };
+    if (tid == 0)
+        for (int k = 0; k < D && k < K; ++k) issue(k);
+
+    F2Win w;
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            w.W[i][r] = make_uint4(0, 0, 0, 0);
+            w.B[i][r] = make_uint4(0, 0, 0, 0);
+        }
+    int z = zs - 3;                        // plane of the black update (even)
+    if (z < 0) z += L;
+    int k = 0;
+
+#define F2_STEP(PH, O)                                                        \
+    {                                                                         \
+        if (k >= K) break;                                                    \
+        f2_step<R4, PLANE, PH, O>(w, c, k, z, keys);                          \
+        __syncthreads();                                                      \
+        if (tid == 0 && k + D < K) {                                          \
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      \
+            issue(k + D);                                                     \
+        }                                                                     \
+        ++k;                                                                  \
+        z = (z + 1 == L) ? 0 : z + 1;                                         \
+    }
+    for (;;) {
+        F2_STEP(0, 0)
+        F2_STEP(1, 1)
+        F2_STEP(2, 0)
+        F2_STEP(0, 1)
+        F2_STEP(1, 0)
+        F2_STEP(2, 1)
+    }
+#undef F2_STEP
+}
+
+// ---------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------
+inline bool fused2_supported(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096; }
+
+template <int R4, int NT>
+inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L,
+                                   const SweepConsts &keys, int sm_count, cudaStream_t stream)
+{
+    constexpr int TY = 2 * NT / R4;
+    constexpr int PLANE = TY * R4;
+    constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
+    static int plan_L = 0, plan_sms = 0, nty = 0, RPT = 0, nzc = 0;
+    if (plan_L != L || plan_sms != sm_count) {
+        cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        int occ = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT>, NT, smem);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
+        const int tyo = TY - 4;                        // stored rows per tile (even)
+        nty = (L + tyo - 1) / tyo;
+        RPT = (L + nty - 1) / nty;
+        RPT += RPT & 1;                                // even, so that ybase is even
+        nty = (L + RPT - 1) / RPT;
+        nzc = (sm_count * occ) / nty;
+        if (nzc < 1) nzc = 1;
+        if (nzc > L / 8) nzc = L / 8;
+        plan_L = L;
+        plan_sms = sm_count;
+    }
+    dim3 grid((unsigned)nty, (unsigned)nzc);
+    fused2_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(
+        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, RPT, nzc, keys);
+    return cudaGetLastError();
+}
+
+inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
+                                       uint64_t seed, int sm_count, cudaStream_t stream)
+{
+    const SweepConsts keys = make_sweep_consts(seed, t);
+    switch (L) {
+        case 512:  return launch_fused2_t<2, 128>(src, dst, L, keys, sm_count, stream);
+        case 1024: return launch_fused2_t<4, 256>(src, dst, L, keys, sm_count, stream);
+        case 2048: return launch_fused2_t<8, 256>(src, dst, L, keys, sm_count, stream);
+        case 4096: return launch_fused2_t<16, 256>(src, dst, L, keys, sm_count, stream);
+        default:   return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace ising
