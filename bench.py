@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=2048)
     ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (throughput window)")
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-measure", action="store_true", help="step = reset + sweeps only")
@@ -200,7 +200,7 @@ def run_ours(args):
     L, S = args.L, args.sweeps
     seed = 4 + rank                                   # config 5: seed 4 (replica r: 4 + r)
     variant = {"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
-               "fused": binding.VARIANT_FUSED}[args.variant]
+               "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2}[args.variant]
     sim = binding.Ising3D(L, [seed], variant=variant)
     N = L ** 3
     n_words = N // 32
@@ -283,8 +283,9 @@ def run_ours(args):
 
     # ---------------- roofline of the dominant kernel (the sweep kernel) ----------------
     peak, peak_src, peaks = measured_peak()
-    kernel = "fused_sweep_kernel" if sim.variant_name == "fused" else "halfsweep_generic_kernel"
-    launches_per_sweep = 1 if sim.variant_name == "fused" else 2
+    kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel"}.get(
+        sim.variant_name, "halfsweep_generic_kernel")
+    launches_per_sweep = 1 if sim.variant_name in ("fused", "fused2") else 2
     avg_launch_ms = sweep_ms / (S * launches_per_sweep)
     algo_bytes_per_launch = ALGO_BYTES_PER_SITE_UPDATE * N / launches_per_sweep
     achieved = algo_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9

@@ -2,6 +2,7 @@
 // No CPU fallback anywhere: every compute entry point launches CUDA kernels or fails.
 #include "../../include/ising3d.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -221,13 +222,6 @@ void postprocess(int L, uint64_t n_up, const uint64_t *antipar, double c_interce
     }
 }
 
-int pow2_floor(int v)
-{
-    int p = 1;
-    while (2 * p <= v) p *= 2;
-    return p;
-}
-
 }  // namespace
 
 extern "C" {
@@ -309,7 +303,7 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
         return fail(ISING3D_EINVAL, "measurement record shape does not match the handle");
     if (!out->n_up || !out->n_broken || !out->antipar)
         return fail(ISING3D_EINVAL, "n_up, n_broken and antipar must be provided");
-    const int L = h->L, WPR = L >> 6, nr = L / 2 + 1, cpr = h->counts_per_replica();
+    const int L = h->L, nr = L / 2 + 1, cpr = h->counts_per_replica();
     const uint32_t *st = h->state[h->cur];
     CUDA_TRY(cudaMemsetAsync(h->d_counts, 0, (size_t)h->n_rep * cpr * 8, h->stream));
     {
@@ -319,27 +313,30 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
             st, h->d_counts, h->words_per_replica(), cpr);
     }
     {
-        // T[2][L][WX] words of shared memory, WX a power of two
-        int WX = pow2_floor(std::max(1, std::min(WPR, 16384 / L)));
-        const int tiles = (WPR + WX - 1) / WX;
-        const size_t smem = (size_t)2 * L * WX * 4;
-        CUDA_TRY(cudaFuncSetAttribute(ising::measure_yz_kernel<1>,
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CUDA_TRY(cudaFuncSetAttribute(ising::measure_yz_kernel<2>,
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        dim3 grid((unsigned)(L * tiles), (unsigned)h->n_rep);
-        ising::measure_yz_kernel<1><<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, WX, tiles, cpr);
-        ising::measure_yz_kernel<2><<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, WX, tiles, cpr);
-    }
-    {
-        // T[2][RX][WPR]; RX rows per block, RX divides L*L
-        int RX = pow2_floor(std::max(1, 8192 / WPR));
-        while (((size_t)L * L) % RX) RX /= 2;
-        const size_t smem = (size_t)2 * RX * WPR * 4;
-        CUDA_TRY(cudaFuncSetAttribute(ising::measure_x_kernel,
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        dim3 grid((unsigned)((size_t)L * L / RX), (unsigned)h->n_rep);
-        ising::measure_x_kernel<<<grid, 512, smem, h->stream>>>(st, h->d_counts, L, RX, cpr);
+        // A_mu(r): persistent CTAs over tiles of C line-word sequences (kernels_measure.cuh)
+        const int C = ising::autocorr_tile_sequences(L);
+        const int n_tiles = (L * L / 32) / C;
+        const size_t smem = ising::autocorr_smem_bytes(L, C);
+        static bool attr_set = false;
+        if (!attr_set) {
+            const int max_smem = (int)ising::autocorr_smem_bytes(4096, 8) + 4096;
+            CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<0>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+            CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<1>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+            CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<2>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+            attr_set = true;
+        }
+        int gx = std::max(1, (h->sm_count + h->n_rep - 1) / h->n_rep);
+        gx = std::min(gx, n_tiles);
+        dim3 grid((unsigned)gx, (unsigned)h->n_rep);
+        ising::autocorr_kernel<0><<<grid, ising::kAcThreads, smem, h->stream>>>(st, h->d_counts, L, C,
+                                                                                n_tiles, cpr);
+        ising::autocorr_kernel<1><<<grid, ising::kAcThreads, smem, h->stream>>>(st, h->d_counts, L, C,
+                                                                                n_tiles, cpr);
+        ising::autocorr_kernel<2><<<grid, ising::kAcThreads, smem, h->stream>>>(st, h->d_counts, L, C,
+                                                                                n_tiles, cpr);
     }
     h->launches += 4;
     CUDA_TRY(cudaGetLastError());

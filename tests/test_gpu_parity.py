@@ -30,6 +30,11 @@ def orc():
     return oracle
 
 
+def VARIANTS(B):
+    return {"auto": B.VARIANT_AUTO, "generic": B.VARIANT_GENERIC, "fused": B.VARIANT_FUSED,
+            "fused2": B.VARIANT_FUSED2}
+
+
 def check_measure(got, want, rep=0):
     assert int(got["n_up"][rep]) == want["n_up"]
     assert np.array_equal(got["antipar"][rep], want["antipar"])
@@ -99,19 +104,21 @@ def test_config2_L256_full_run(B, orc):
 
 
 # ------------------------------------------------------------------ fused kernel, larger rows
+@pytest.mark.parametrize("variant", ["fused", "fused2"])
 @pytest.mark.parametrize("L,seed,cps", [(512, 11, [1, 2, 4]), (1024, 3, [1, 2])])
-def test_fused_kernel_larger_L(B, orc, L, seed, cps):
+def test_fused_kernel_larger_L(B, orc, L, seed, cps, variant):
     thin = None if L <= 512 else np.array([0, 1, 2, 3, 7, 64, 255, 256, 511, 512], dtype=np.int32)
-    run_against_oracle(B, orc, L, seed, cps, B.VARIANT_FUSED, measure_at={cps[-1]}, thin_r=thin)
+    run_against_oracle(B, orc, L, seed, cps, VARIANTS(B)[variant], measure_at={cps[-1]}, thin_r=thin)
 
 
-@pytest.mark.parametrize("L", [256, 512, 1024, 2048])
-def test_fused_equals_generic(B, L):
-    """Not an oracle check: the two kernels must agree bit for bit (also at sizes and times
+@pytest.mark.parametrize("L,variant", [(256, "fused"), (512, "fused"), (1024, "fused"), (2048, "fused"),
+                                       (512, "fused2"), (1024, "fused2"), (2048, "fused2")])
+def test_fused_equals_generic(B, L, variant):
+    """Not an oracle check: the kernels must agree bit for bit (also at sizes and times
     the oracle cannot reach); the generic kernel is oracle-checked above."""
-    a = B.Ising3D(L, [5], variant=B.VARIANT_FUSED)
+    a = B.Ising3D(L, [5], variant=VARIANTS(B)[variant])
     b = B.Ising3D(L, [5], variant=B.VARIANT_GENERIC)
-    assert a.variant_name == "fused" and b.variant_name == "generic"
+    assert a.variant_name == variant and b.variant_name == "generic"
     for n in (1, 2, 7):
         a.sweep(n)
         b.sweep(n)
@@ -122,13 +129,15 @@ def test_fused_equals_generic(B, L):
 
 # ------------------------------------------------------------------ config 5 (full size, sampled)
 def _sample_sites(L, n, seed, RPT=28):
+    """RPT = stored rows per y tile of the kernel under test (fused: 28, fused2 at L=2048: 60)."""
     rng = np.random.Generator(np.random.PCG64(seed))
     xyz = rng.integers(0, L, size=(n, 3))
     # force the structural edges: row ends / word and group boundaries in x, y-tile borders of
     # the fused kernel (multiples of RPT and the wrap), z-chunk borders and the z wrap
     xs = [0, 1, 2, 63, 64, 65, 255, 256, 257, L // 2 - 1, L // 2, L - 2, L - 1]
     ys = [0, 1, 2, RPT - 2, RPT - 1, RPT, RPT + 1, 2 * RPT - 1, 2 * RPT, L - 3, L - 2, L - 1]
-    zs = [0, 1, 2, 3, L // 6, L // 6 + 1, L // 3, L // 3 + 1, L // 2, L - 3, L - 2, L - 1]
+    zs = [0, 1, 2, 3, L // 6, L // 6 + 1, L // 3, L // 3 + 1, L // 2, L - 3, L - 2, L - 1,
+          L // 8 - 1, L // 8, L // 8 + 1, L // 8 + 2, L // 4, L // 4 + 1]   # fused2: odd chunk borders
     k = 0
     for x in xs:
         for y in ys[::2]:
@@ -152,13 +161,16 @@ def _bits_at(words, L, xyz):
     return np.where((w >> (b & 31).astype(np.uint32)) & 1, 1, -1).astype(np.int8)
 
 
-@pytest.mark.parametrize("L,seed,variant", [(2048, 4, "fused"), (2048, 4, "generic"), (1024, 3, "fused")])
+@pytest.mark.parametrize("L,seed,variant", [(2048, 4, "auto"), (2048, 4, "fused"), (2048, 4, "generic"),
+                                            (1024, 3, "auto")])
 def test_full_size_sampled_sites(B, orc, L, seed, variant):
     """Config 5 / 4 at full size in the launch configuration bench.py times: sampled sites
     after 0, 1 and 2 sweeps against values the oracle computes one by one from the
     definition (light-cone recursion, no GPU data involved)."""
-    sim = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC)
-    xyz = _sample_sites(L, 3000, 17)
+    sim = B.Ising3D(L, [seed], variant=VARIANTS(B)[variant])
+    if variant == "auto":                            # what bench.py launches
+        assert sim.variant_name == "fused2"
+    xyz = _sample_sites(L, 3000, 17, RPT=60 if sim.variant_name == "fused2" else 28)
     buf = np.empty(L ** 3 // 32, dtype=np.uint32)
     for n_sweeps in (0, 1, 2):
         if n_sweeps:
