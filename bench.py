@@ -130,7 +130,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from oracle import oracle as orc
-    L, n_sw, seed = 256, 10, 4
+    L, n_sw, seed = 512, 20, 4
     sample = ("L=%d (config-5 start rule: iid p=1/2 from seed %d), sweeps 0..%d per step; "
               "the oracle cannot hold 1000 sweeps of L=2048 in minutes" % (L, seed, n_sw - 1))
     for _ in range(args.warmup):
@@ -165,13 +165,18 @@ def measured_peak():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)", {}
 
 
-def ncu_traffic(kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
-    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+def ncu_traffic(kernel: str, L: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed ncu --set full capture (profiles/roofline_traffic.csv); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     try:
-        return json.load(open(p)).get(kernel)
+        for line in open(p).read().splitlines()[1:]:
+            k, l, b, _ = line.split(",")
+            if k == kernel and int(l) == L:
+                return float(b)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def run_ours(args):
@@ -297,7 +302,7 @@ def run_ours(args):
     hbm_bound = peak / ALGO_BYTES_PER_SITE_UPDATE
     roofline = {
         "bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": achieved / peak, "traffic": ncu_traffic(kernel),
+        "frac": achieved / peak, "traffic": ncu_traffic(kernel, L),
         "algorithmic_bytes_per_launch": algo_bytes_per_launch, "avg_launch_ms": avg_launch_ms,
         "peak_source": peak_src,
         "sweep_only_site_updates_per_ns": N * S / (sweep_ms * 1e6),
@@ -310,7 +315,7 @@ def run_ours(args):
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        Lc, nsw = 512, 12
+        Lc, nsw = 1024, 16                          # ~1.7e10 site-updates: 10-30 s on 8-16 cores
         rate, dt, cores = oracle_rate(Lc, nsw, 4)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "L=%d, iid p=1/2 start from seed 4, sweeps 0..%d (%.1f s of CPU work); "
