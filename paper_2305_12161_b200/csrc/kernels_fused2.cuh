@@ -254,28 +254,34 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     }
     __syncthreads();
 
-    // producer: stage k holds W_old[z0+1+k] and B_old[z0+k], z0 = zs-3 (periodic)
+    // producer (thread 0): stage k holds W_old[z0+1+k] and B_old[z0+k], z0 = zs-3 (periodic).
+    // Stages are issued in order, so the plane indices and pointers advance incrementally
+    // (no division in the loop).  No proxy fence is needed before re-filling a stage: its last
+    // generic-proxy accesses were loads that completed before the __syncthreads.
     const int n1 = min(TY, L - ybase);     // rows before the periodic wrap in y
-    auto issue = [&](int k) {
-        const int s = k & (S - 1);
-        int zw = zs - 2 + k;
-        zw = (zw % L + L) % L;
-        int zb = zs - 3 + k;
-        zb = (zb % L + L) % L;
+    const uint32_t bytes1 = (uint32_t)n1 * R4 * 16u, bytes2 = (uint32_t)(TY - n1) * R4 * 16u;
+    const size_t plane_u4 = (size_t)L * R4;
+    int pzw = ((zs - 2) % L + L) % L, pzb = ((zs - 3) % L + L) % L, pk = 0;
+    const uint4 *pgw = src + G + (size_t)pzw * plane_u4;
+    const uint4 *pgb = src + (size_t)pzb * plane_u4;
+    auto issue_next = [&]() {
+        const int s = pk & (S - 1);
         const uint32_t bar = smem_u32(&bars[s]);
-        const uint32_t bytes = (uint32_t)PLANE * 16u;
-        mbar_expect_tx(bar, 2 * bytes);
-        const uint4 *gw = src + G + ((size_t)zw * L) * R4;
-        const uint4 *gb = src + ((size_t)zb * L) * R4;
-        bulk_g2s(smem_u32(Wst + s * PLANE), gw + (size_t)ybase * R4, (uint32_t)n1 * R4 * 16u, bar);
-        bulk_g2s(smem_u32(Bst + s * PLANE), gb + (size_t)ybase * R4, (uint32_t)n1 * R4 * 16u, bar);
-        if (n1 < TY) {
-            bulk_g2s(smem_u32(Wst + s * PLANE + n1 * R4), gw, (uint32_t)(TY - n1) * R4 * 16u, bar);
-            bulk_g2s(smem_u32(Bst + s * PLANE + n1 * R4), gb, (uint32_t)(TY - n1) * R4 * 16u, bar);
+        mbar_expect_tx(bar, 2u * (uint32_t)PLANE * 16u);
+        bulk_g2s(smem_u32(Wst + s * PLANE), pgw + (size_t)ybase * R4, bytes1, bar);
+        bulk_g2s(smem_u32(Bst + s * PLANE), pgb + (size_t)ybase * R4, bytes1, bar);
+        if (bytes2) {
+            bulk_g2s(smem_u32(Wst + s * PLANE + n1 * R4), pgw, bytes2, bar);
+            bulk_g2s(smem_u32(Bst + s * PLANE + n1 * R4), pgb, bytes2, bar);
         }
+        ++pk;
+        pgw += plane_u4;
+        pgb += plane_u4;
+        if (++pzw == L) { pzw = 0; pgw = src + G; }
+        if (++pzb == L) { pzb = 0; pgb = src; }
     };
     if (tid == 0)
-        for (int k = 0; k < D && k < K; ++k) issue(k);
+        for (int k = 0; k < D && k < K; ++k) issue_next();
 
     F2Win w;
 #pragma unroll
@@ -294,10 +300,7 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
         if (k >= K) break;                                                    \
         f2_step<R4, PLANE, PH, O>(w, c, k, z, keys);                          \
         __syncthreads();                                                      \
-        if (tid == 0 && k + D < K) {                                          \
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      \
-            issue(k + D);                                                     \
-        }                                                                     \
+        if (tid == 0 && pk < K) issue_next();                                 \
         ++k;                                                                  \
         z = (z + 1 == L) ? 0 : z + 1;                                         \
     }
