@@ -76,6 +76,8 @@ extern "C" {
 #define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
 #define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
 #define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096)        */
+#define ISING3D_VARIANT_RESIDENT 4  /* lattice resident in the shared memory of a thread-block
+                                       cluster, all sweeps of a call in one launch (L in 64..256) */
 
 typedef struct ising3d ising3d_t;   /* opaque */
 
@@ -173,6 +175,9 @@ uint64_t ising3d_sweep_count(const ising3d_t *h);
 uint64_t ising3d_launch_count(const ising3d_t *h);
 /* name of the sweep kernel the handle currently dispatches to ("generic", "fused", ...) */
 const char *ising3d_variant_name(const ising3d_t *h);
+/* CTAs per thread-block cluster (= SMs per lattice) of the resident kernel; 0 if another
+ * kernel is dispatched. */
+int ising3d_cluster_size(const ising3d_t *h);
 
 /* Block until all work queued on the handle's stream is done. */
 int ising3d_sync(ising3d_t *h);

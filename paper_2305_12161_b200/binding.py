@@ -17,14 +17,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libising3d.so")
 
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
-VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2 = 0, 1, 2, 3
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT = 0, 1, 2, 3, 4
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
     "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant",
     "ising3d_sweep", "ising3d_measure", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
-    "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_sync",
+    "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size", "ising3d_sync",
     "ising3d_free", "ising3d_last_error",
 ]
 
@@ -76,6 +76,7 @@ def load():
         "ising3d_sweep_count": (u64, [vp]),
         "ising3d_launch_count": (u64, [vp]),
         "ising3d_variant_name": (C.c_char_p, [vp]),
+        "ising3d_cluster_size": (C.c_int, [vp]),
         "ising3d_sync": (C.c_int, [vp]),
         "ising3d_free": (None, [vp]),
         "ising3d_last_error": (C.c_char_p, []),
@@ -176,6 +177,10 @@ class Ising3D:
     @property
     def launch_count(self) -> int:
         return int(self._l.ising3d_launch_count(self._h))
+
+    @property
+    def cluster_size(self) -> int:
+        return int(self._l.ising3d_cluster_size(self._h))
 
     @property
     def variant_name(self) -> str:

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -16,6 +17,7 @@
 #include "kernels_fused2.cuh"
 #include "kernels_generic.cuh"
 #include "kernels_measure.cuh"
+#include "kernels_resident.cuh"
 #include "philox.cuh"
 
 namespace {
@@ -56,12 +58,34 @@ struct ising3d {
     int variant = ISING3D_VARIANT_AUTO;
     uint64_t launches = 0;
     int sm_count = 148;
+    mutable ising::ResidentPlan res_plan = {0, 0};
+    mutable bool res_planned = false;
 
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
     int counts_per_replica() const { return 1 + 3 * (L / 2 + 1); }
     bool fused_ok() const { return n_rep == 1 && ising::fused_supported(L); }
     bool fused2_ok() const { return n_rep == 1 && ising::fused2_supported(L); }
+    bool resident_ok() const
+    {
+        if (!ising::resident_supported(L)) return false;
+        if (!res_planned) {
+            res_plan = ising::resident_plan(L, n_rep, sm_count);
+            if (const char *e = getenv("ISING3D_RESIDENT_CS")) {     // experiments only
+                const int cs = atoi(e);
+                if (cs >= 1 && cs <= 16 && L % cs == 0 && L / cs >= 2 &&
+                    ising::resident_smem_bytes(L, cs) <= 200 * 1024)
+                    res_plan = ising::ResidentPlan{cs, ising::resident_smem_bytes(L, cs)};
+            }
+            res_planned = true;
+        }
+        return res_plan.cs > 0;
+    }
+    bool use_resident() const
+    {
+        return variant == ISING3D_VARIANT_RESIDENT ||
+               (variant == ISING3D_VARIANT_AUTO && resident_ok());
+    }
     bool use_fused2() const
     {
         return variant == ISING3D_VARIANT_FUSED2 || (variant == ISING3D_VARIANT_AUTO && fused2_ok());
@@ -69,7 +93,7 @@ struct ising3d {
     bool use_fused() const
     {
         return variant == ISING3D_VARIANT_FUSED ||
-               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok());
+               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok() && !resident_ok());
     }
 };
 
@@ -176,6 +200,16 @@ int sweep_generic(ising3d *h, uint64_t n)
     return ISING3D_OK;
 }
 
+int sweep_resident(ising3d *h, uint64_t n)
+{
+    cudaError_t e = ising::launch_resident(h->state[h->cur], h->d_seeds, h->L, h->n_rep, h->res_plan,
+                                           (uint32_t)h->sweep, (uint32_t)n, h->stream);
+    if (e != cudaSuccess)
+        return fail(ISING3D_ECUDA, std::string("resident sweep launch: ") + cudaGetErrorString(e));
+    h->launches += 1;
+    return ISING3D_OK;
+}
+
 int sweep_fused(ising3d *h, uint64_t n, bool gen2)
 {
     const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
@@ -272,12 +306,14 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream)
 int ising3d_set_variant(ising3d_t *h, int variant)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED2)
+    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_RESIDENT)
         return fail(ISING3D_EINVAL, "unknown variant");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
         return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())
         return fail(ISING3D_EINVAL, "fused2 kernel needs n_rep == 1 and L in {512,1024,2048,4096}");
+    if (variant == ISING3D_VARIANT_RESIDENT && !h->resident_ok())
+        return fail(ISING3D_EINVAL, "resident kernel needs L in {64,128,256} and a cluster that fits");
     h->variant = variant;
     return ISING3D_OK;
 }
@@ -288,7 +324,8 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xFFFFFFFFull || h->sweep + n_sweeps < h->sweep)
         return fail(ISING3D_EINVAL, "sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return ISING3D_OK;
-    const int rc = h->use_fused2()  ? sweep_fused(h, n_sweeps, true)
+    const int rc = h->use_resident() ? sweep_resident(h, n_sweeps)
+                   : h->use_fused2()  ? sweep_fused(h, n_sweeps, true)
                    : h->use_fused() ? sweep_fused(h, n_sweeps, false)
                                     : sweep_generic(h, n_sweeps);
     if (rc != ISING3D_OK) return rc;
@@ -410,7 +447,12 @@ uint64_t ising3d_launch_count(const ising3d_t *h) { return h ? h->launches : 0; 
 const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";
-    return h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
+    return h->use_resident() ? "resident" : h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
+}
+
+int ising3d_cluster_size(const ising3d_t *h)
+{
+    return (h && h->use_resident()) ? h->res_plan.cs : 0;
 }
 
 int ising3d_sync(ising3d_t *h)

@@ -34,7 +34,7 @@ def ell_from_C(C: np.ndarray, c: float = 0.5) -> float:
     return float("nan")
 
 
-def run_workload(name: str, max_sweeps: int | None, emit):
+def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto"):
     import torch
     from . import binding
 
@@ -44,7 +44,9 @@ def run_workload(name: str, max_sweeps: int | None, emit):
     times = [t for t in w["times"] if t <= n_total]
     if not times or times[-1] != n_total:
         times.append(n_total)
-    sim = binding.Ising3D(L, seeds)
+    sim = binding.Ising3D(L, seeds, variant={"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
+                                             "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2,
+                                             "resident": binding.VARIANT_RESIDENT}[variant])
     N = L ** 3 * len(seeds)
     ev = lambda: torch.cuda.Event(enable_timing=True)
     t_sweeps = t_meas = 0.0
@@ -74,7 +76,7 @@ def run_workload(name: str, max_sweeps: int | None, emit):
     e_all1 = ev(); e_all1.record(); torch.cuda.synchronize()
     total_ms = e_all0.elapsed_time(e_all1)
     summary = {"workload": name, "summary": True, "L": L, "replicas": len(seeds), "sweeps": n_total,
-               "checkpoints": len(times), "kernel": sim.variant_name,
+               "checkpoints": len(times), "kernel": sim.variant_name, "cluster_size": sim.cluster_size,
                "site_updates_per_ns_sweeps": N * n_total / (t_sweeps * 1e6),
                "site_updates_per_ns_total": N * n_total / (total_ms * 1e6),
                "ms_sweeps": t_sweeps, "ms_measure": t_meas, "ms_total": total_ms,
@@ -90,6 +92,8 @@ def main(argv=None):
     ap.add_argument("--configs", default=",".join(inputs.WORKLOADS))
     ap.add_argument("--max-sweeps", type=int, default=None,
                     help="truncate each workload to this many sweeps (default: the full run)")
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "resident"],
+                    help="sweep kernel (default: the library's choice)")
     ap.add_argument("--out", default=None, help="also append the JSON lines to this file")
     args = ap.parse_args(argv)
     from . import build
@@ -104,7 +108,7 @@ def main(argv=None):
             fh.flush()
 
     for name in args.configs.split(","):
-        run_workload(name.strip(), args.max_sweeps, emit)
+        run_workload(name.strip(), args.max_sweeps, emit, args.variant)
     return 0
 
 

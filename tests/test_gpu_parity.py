@@ -32,7 +32,7 @@ def orc():
 
 def VARIANTS(B):
     return {"auto": B.VARIANT_AUTO, "generic": B.VARIANT_GENERIC, "fused": B.VARIANT_FUSED,
-            "fused2": B.VARIANT_FUSED2}
+            "fused2": B.VARIANT_FUSED2, "resident": B.VARIANT_RESIDENT}
 
 
 def check_measure(got, want, rep=0):
@@ -81,6 +81,38 @@ def test_config1_L64_all_checkpoints(B, orc):
 def test_generic_kernel_other_sizes(B, orc, L, seed, cps):
     """Rows of 2, 3 and 5 words: ragged measurement tiles, non-power-of-two rows."""
     run_against_oracle(B, orc, L, seed, cps, B.VARIANT_GENERIC)
+
+
+# ------------------------------------------------------------------ resident (cluster) kernel
+@pytest.mark.parametrize("L,cs,seed,cps", [(64, 1, 1, [1, 2, 5, 10]), (64, 2, 1, [3, 10]), (64, 8, 21, [1, 7]),
+                                           (64, 16, 22, [2, 5]), (128, 2, 7, [1, 2, 5, 12]), (128, 4, 7, [3, 12]),
+                                           (128, 8, 23, [1, 6]), (128, 16, 24, [4]), (256, 16, 2, [1, 3, 10])])
+def test_resident_kernel_cluster_sizes(B, orc, L, cs, seed, cps, monkeypatch):
+    """The shared-memory-resident multi-sweep kernel at every cluster size (z slabs of L/cs
+    planes, halo planes exchanged through distributed shared memory), against the oracle."""
+    monkeypatch.setenv("ISING3D_RESIDENT_CS", str(cs))
+    sim = B.Ising3D(L, [seed], variant=B.VARIANT_RESIDENT)
+    assert sim.variant_name == "resident" and sim.cluster_size == cs
+    ref = orc.Oracle(L, seed)
+    t = 0
+    for cp in cps:
+        sim.sweep(cp - t)
+        ref.sweep(cp - t)
+        t = cp
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+    check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+
+
+def test_resident_is_the_default_for_small_lattices(B):
+    a = B.Ising3D(64, [1])
+    b = B.Ising3D(128, list(range(100, 164)))
+    c = B.Ising3D(256, [2])
+    assert a.variant_name == "resident" and b.variant_name == "resident"
+    assert c.variant_name in ("resident", "fused")      # resident needs a 16-CTA cluster
+    assert a.cluster_size >= 1 and b.cluster_size * 64 <= 148
+    for s in (a, b, c):
+        s.free()
 
 
 # ------------------------------------------------------------------ config 2
@@ -217,10 +249,11 @@ def test_L2048_measurement_closed_form(B):
 
 
 # ------------------------------------------------------------------ config 3 (batch)
-def test_config3_batch_equals_singles_and_oracle(B, orc):
+@pytest.mark.parametrize("variant", ["auto", "generic"])
+def test_config3_batch_equals_singles_and_oracle(B, orc, variant):
     L = 128
     seeds = inputs.WORKLOADS["config3_64xL128"]["seeds"]
-    batch = B.Ising3D(L, seeds)
+    batch = B.Ising3D(L, seeds, variant=VARIANTS(B)[variant])
     assert batch.n_rep == 64
     wpr = L ** 3 // 32
     cps = [1, 2, 5, 20]
@@ -247,9 +280,10 @@ def test_config3_batch_equals_singles_and_oracle(B, orc):
 
 
 # ------------------------------------------------------------------ set_state / structured inputs
-@pytest.mark.parametrize("L,variant", [(64, "generic"), (128, "generic"), (256, "fused"), (256, "generic")])
+@pytest.mark.parametrize("L,variant", [(64, "generic"), (128, "generic"), (256, "fused"), (256, "generic"),
+                                       (64, "resident"), (128, "resident")])
 def test_set_state_random_and_coarse_inputs(B, orc, L, variant):
-    v = B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC
+    v = VARIANTS(B)[variant]
     for words, t0 in [(inputs.random_words(L, 1, 123), 0), (inputs.coarse_words(L, 5), 1000),
                       (inputs.coarse_words(L, 6, block=16), 4_000_000_000)]:
         sim = B.Ising3D(L, [77], variant=v)
@@ -265,11 +299,11 @@ def test_set_state_random_and_coarse_inputs(B, orc, L, variant):
         sim.free()
 
 
-@pytest.mark.parametrize("variant", ["generic", "fused"])
+@pytest.mark.parametrize("variant", ["generic", "fused", "resident"])
 def test_structured_states(B, orc, variant):
     """Fixed points, Neel state, single spins and 2x2x2 cubes across every periodic wrap."""
     L = 256 if variant == "fused" else 64
-    v = B.VARIANT_FUSED if variant == "fused" else B.VARIANT_GENERIC
+    v = VARIANTS(B)[variant]
     states = [inputs.all_up(L), -inputs.all_up(L), inputs.neel(L), -inputs.neel(L)]
     for axis in (0, 1, 2):
         states.append(inputs.slab(L, axis, L - 1, 2))
@@ -315,6 +349,8 @@ def test_checkpoint_resume_and_reset(B, orc):
 
 def test_library_owned_memory_and_errors(B, orc):
     sim = B.Ising3D(64, [1], torch_buffer=False)
+    with pytest.raises(B.Ising3DError):
+        B.Ising3D(512, [1], variant=B.VARIANT_RESIDENT)   # does not fit any cluster
     ref = orc.Oracle(64, 1)
     sim.sweep(2)
     ref.sweep(2)
