@@ -32,6 +32,11 @@
  *   orc_postprocess     : closed forms, hand-worked example
  *   orc_export/import   : round trip, independent Python packer
  *   orc_site_after      : equals orc_sweep site by site on small L
+ *   orc_first_colour / orc_sweep_mixed : Neel state closed form (the first colour
+ *                         decides the sign of the ordered state), bit statistics,
+ *                         big-integer Python Philox
+ *   orc_menger_solid / orc_init_menger : solid counts 20^k, the k = 1 cross written
+ *                         out, self-similarity, tile-sign statistics, k = 0 iid
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -233,6 +238,84 @@ void orc_sweep(orc_t *o, uint64_t n_sweeps)
         orc_half_sweep(o, o->sweep, 1, 0, 0);
         o->sweep += 1;
     }
+}
+
+/* ------------------------------------------------------------------ */
+/* Mixed cycle (Supp. I.B PAPER.md:258): "choosing at */
+/* random which sublattice to update first ... still every spin is      */
+/* proposed to flip exactly once per sweep".  Reading D10: the first    */
+/* colour of sweep t is bit 0 of word 0 of Philox(key = seed, counter = */
+/* (0, t, 0, tag = 2)); the tie bits keep counter (q, t, c, 0) with c   */
+/* the colour being updated.                                            */
+/* ------------------------------------------------------------------ */
+int orc_first_colour(uint64_t seed, uint32_t t)
+{
+    uint32_t ctr[4] = { 0u, t, 0u, 2u };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    orc_philox4x32_10(ctr, key, out);
+    return (int)(out[0] & 1u);
+}
+
+void orc_sweep_mixed(orc_t *o, uint64_t n_sweeps)
+{
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        int first = orc_first_colour(o->seed, o->sweep);
+        orc_half_sweep(o, o->sweep, first, 0, 0);
+        orc_half_sweep(o, o->sweep, 1 - first, 0, 0);
+        o->sweep += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* Menger-sponge start: "The starting   */
+/* configuration of dimensions L^3 is created by repeating sponges of   */
+/* k-th iteration of size (3^k)^3.  For each sponge we pick uniformly   */
+/* at random whether the Menger structure is represented by up or down  */
+/* spins."  A site with local coordinates (u,v,w) in [0,3^k)^3 belongs  */
+/* to the k-th iteration sponge iff at no ternary digit position two or */
+/* more of u, v, w have the digit 1 (the removed cross of each 3x3x3).  */
+/* Reading D11: tiles start at the origin, the last tile in each        */
+/* direction is cut off at L (L need not be a multiple of 3^k, cf.      */
+/* Fig. 4(b): 128^3 from 27^3 sponges); tile (X,Y,Z) has    */
+/* linear index T = (Z*nT + Y)*nT + X, nT = ceil(L/3^k); its sign bit   */
+/* is bit (T & 31) of word ((T >> 5) & 3) of Philox(key = seed, counter */
+/* = (T >> 7, k, 0, tag = 3)); sponge sites get +1 if the bit is 1,     */
+/* holes the opposite sign.  k = 0 gives one site per tile: an iid      */
+/* p = 1/2 start ("k = 0 (corresponding to our case from    */
+/* before)").                                                           */
+/* ------------------------------------------------------------------ */
+int orc_menger_solid(int u, int v, int w, int k)
+{
+    for (int level = 0; level < k; ++level) {
+        int ones = (u % 3 == 1) + (v % 3 == 1) + (w % 3 == 1);
+        if (ones >= 2) return 0;
+        u /= 3; v /= 3; w /= 3;
+    }
+    return 1;
+}
+
+void orc_init_menger(orc_t *o, int k)
+{
+    const int L = o->L;
+    int size = 1;
+    for (int i = 0; i < k; ++i) size *= 3;
+    const int nT = (L + size - 1) / size;
+    uint32_t key[2] = { (uint32_t)(o->seed & 0xFFFFFFFFu), (uint32_t)(o->seed >> 32) };
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                uint64_t T = ((uint64_t)(z / size) * (uint64_t)nT + (uint64_t)(y / size)) * (uint64_t)nT
+                           + (uint64_t)(x / size);
+                uint32_t ctr[4] = { (uint32_t)(T >> 7), (uint32_t)k, 0u, 3u };
+                uint32_t out[4];
+                orc_philox4x32_10(ctr, key, out);
+                int bit = (int)((out[(T >> 5) & 3] >> (T & 31)) & 1u);
+                int sign = bit ? 1 : -1;
+                int solid = orc_menger_solid(x % size, y % size, z % size, k);
+                o->s[orc_idx(o, x, y, z)] = (int8_t)(solid ? sign : -sign);
+            }
+    o->sweep = 0;
 }
 
 /* ------------------------------------------------------------------ */

@@ -88,6 +88,14 @@ def lib():
         l.orc_sites_after.argtypes = [C.c_uint64, C.c_int, i32p, C.c_int, C.c_int,
                                       C.POINTER(C.c_int8)]
         l.orc_sites_after.restype = None
+        l.orc_first_colour.argtypes = [C.c_uint64, C.c_uint32]
+        l.orc_first_colour.restype = C.c_int
+        l.orc_sweep_mixed.argtypes = [C.c_void_p, C.c_uint64]
+        l.orc_sweep_mixed.restype = None
+        l.orc_menger_solid.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
+        l.orc_menger_solid.restype = C.c_int
+        l.orc_init_menger.argtypes = [C.c_void_p, C.c_int]
+        l.orc_init_menger.restype = None
         l.orc_num_threads.argtypes = []
         l.orc_num_threads.restype = C.c_int
         l.orc_set_num_threads.argtypes = [C.c_int]
@@ -121,6 +129,16 @@ def sites_after(seed, L, xyz, n_half_sweeps):
     lib().orc_sites_after(int(seed), int(L), _p(a, C.c_int32), len(a), int(n_half_sweeps),
                           _p(out, C.c_int8))
     return out
+
+
+def first_colour(seed: int, t: int) -> int:
+    """Mixed cycle (D10): the colour updated first in sweep t."""
+    return int(lib().orc_first_colour(int(seed), int(t)))
+
+
+def menger_solid(u: int, v: int, w: int, k: int) -> int:
+    """1 iff (u,v,w) in [0,3^k)^3 belongs to the k-th iteration Menger sponge."""
+    return int(lib().orc_menger_solid(int(u), int(v), int(w), int(k)))
 
 
 def num_threads() -> int:
@@ -197,6 +215,14 @@ class Oracle:
 
     def sweep(self, n: int = 1):
         self._l.orc_sweep(self._h, int(n))
+
+    def sweep_mixed(self, n: int = 1):
+        """n sweeps of the mixed cycle (D10): the first colour is drawn per sweep."""
+        self._l.orc_sweep_mixed(self._h, int(n))
+
+    def init_menger(self, k: int):
+        """Menger-sponge start of iteration k (D11); sweep counter 0."""
+        self._l.orc_init_menger(self._h, int(k))
 
     def half_sweep_brute(self, t: int, c: int):
         self._l.orc_half_sweep_brute(self._h, int(t), int(c))

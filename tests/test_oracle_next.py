@@ -1,0 +1,172 @@
+"""Pins of the oracle functions behind the SURVEY.md 8(f) rows built so far:
+  f-2  mixed cycle (Supp. I.B PAPER.md:258)  -> orc_first_colour, orc_sweep_mixed
+  f-3  Menger-sponge start     -> orc_menger_solid, orc_init_menger
+Each pin is something the paper or the mathematics fixes, not a retyping of the oracle."""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2305_12161_b200 import inputs
+from test_oracle_pins import py_philox, MASK
+
+
+# ------------------------------------------------------------------ f-2: mixed cycle
+def test_first_colour_is_the_documented_philox_bit():
+    """D10: bit 0 of word 0 of Philox(key = seed, counter = (0, t, 0, 2)), against the
+    big-integer Python Philox (itself pinned by the known-answer vectors)."""
+    for seed in (1, 4, 0xDEADBEEFCAFE1234):
+        for t in list(range(40)) + [2 ** 31, 2 ** 32 - 2]:
+            want = py_philox([0, t, 0, 2], [seed & MASK, seed >> 32])[0] & 1
+            assert orc.first_colour(seed, t) == want
+
+
+def test_mixed_cycle_neel_closed_form():
+    """From the Neel state s = (-1)^(x+y+z) the colour updated first flips completely (n = 6)
+    and the lattice orders with the OTHER colour's value (pinned for the
+    fixed order in test_oracle_pins): black first -> all -1, white first -> all +1.  So one
+    mixed sweep from the Neel state reads out the order the oracle really used."""
+    L, seed = 8, 11
+    seen = set()
+    for t in range(48):
+        o = orc.Oracle(L, seed, init=False)
+        o.spins[...] = inputs.neel(L)
+        o.sweep_count = t
+        o.sweep_mixed(1)
+        first = py_philox([0, t, 0, 2], [seed & MASK, seed >> 32])[0] & 1
+        assert np.all(o.spins == (1 if first else -1)), "sweep %d" % t
+        assert o.sweep_count == t + 1
+        seen.add(first)
+    assert seen == {0, 1}
+
+
+def test_mixed_cycle_order_is_fair_and_seed_dependent():
+    n = 4000
+    f1 = np.array([orc.first_colour(5, t) for t in range(n)])
+    f2 = np.array([orc.first_colour(6, t) for t in range(n)])
+    assert abs(f1.sum() - n / 2) < 4 * np.sqrt(n) / 2          # binomial 4 sigma
+    assert abs((f1 != f2).sum() - n / 2) < 4 * np.sqrt(n) / 2  # independent streams
+
+
+def test_mixed_cycle_every_site_proposed_once_and_energy_monotone():
+    """PAPER.md:258 "still every spin is proposed to flip exactly once per sweep": a mixed
+    sweep equals the two half-sweeps of the drawn order, the interface energy never increases
+    (each half-sweep only accepts Delta E <= 0), and a sweep whose drawn order is (0, 1) equals
+    the 01-cycle sweep."""
+    L, seed = 12, 3
+    a = orc.Oracle(L, seed)
+    b = orc.Oracle(L, seed)
+    c = orc.Oracle(L, seed)
+    e_prev = a.measure([1])[1].sum()
+    for t in range(12):
+        first = orc.first_colour(seed, t)
+        state_before = a.spins.copy()
+        a.sweep_mixed(1)
+        b.half_sweep(t, first)
+        b.half_sweep(t, 1 - first)
+        assert np.array_equal(a.spins, b.spins)
+        e = a.measure([1])[1].sum()
+        assert e <= e_prev
+        e_prev = e
+        c.spins[...] = state_before
+        c.sweep_count = t
+        c.sweep(1)
+        if first == 0:
+            assert np.array_equal(c.spins, a.spins)
+
+
+def test_mixed_cycle_fixed_points():
+    L = 8
+    for s0 in (inputs.all_up(L), -inputs.all_up(L), inputs.slab(L, 2, 1, 4)):
+        o = orc.Oracle(L, 9, init=False)
+        o.spins[...] = s0
+        o.sweep_mixed(5)
+        assert np.array_equal(o.spins, s0)
+
+
+# ------------------------------------------------------------------ f-3: Menger sponge
+def test_menger_solid_counts_and_first_iteration():
+    """A k-th iteration Menger sponge keeps 20 of 27 sub-cubes per level: 20^k sites of 27^k.
+    k = 1 written out: of the 27 cells the 6 face centres and the body centre are removed."""
+    for k in range(0, 4):
+        n = 3 ** k
+        cnt = sum(orc.menger_solid(u, v, w, k) for u in range(n) for v in range(n) for w in range(n))
+        assert cnt == 20 ** k
+    removed = {(1, 1, 0), (1, 1, 2), (1, 0, 1), (1, 2, 1), (0, 1, 1), (2, 1, 1), (1, 1, 1)}
+    for u in range(3):
+        for v in range(3):
+            for w in range(3):
+                assert orc.menger_solid(u, v, w, 1) == (0 if (u, v, w) in removed else 1)
+
+
+def test_menger_solid_self_similarity_and_symmetry():
+    """Iteration k+1 = 20 copies of iteration k placed on the iteration-1 pattern; the sponge is
+    invariant under permutations and reflections of the axes."""
+    k = 2
+    n = 3 ** k
+    for u in range(3 * n):
+        for v in range(0, 3 * n, 2):
+            for w in range(0, 3 * n, 3):
+                want = orc.menger_solid(u // n, v // n, w // n, 1) and orc.menger_solid(u % n, v % n, w % n, k)
+                assert orc.menger_solid(u, v, w, k + 1) == int(bool(want))
+    m = 27
+    for (u, v, w) in [(1, 4, 13), (0, 0, 0), (13, 13, 2), (26, 1, 1), (9, 10, 12), (4, 22, 16)]:
+        ref = orc.menger_solid(u, v, w, 3)
+        assert orc.menger_solid(v, w, u, 3) == ref and orc.menger_solid(w, v, u, 3) == ref
+        assert orc.menger_solid(m - 1 - u, v, w, 3) == ref and orc.menger_solid(u, m - 1 - v, m - 1 - w, 3) == ref
+
+
+@pytest.mark.parametrize("L,k", [(54, 3), (32, 2), (20, 1)])
+def test_init_menger_structure(L, k):
+    """Every (possibly cut) tile is one sponge pattern or its negative, the pattern
+    is the restated Menger rule, and the sign is the documented Philox bit (D11)."""
+    size = 3 ** k
+    seed = 77
+    o = orc.Oracle(L, seed, init=False)
+    o.init_menger(k)
+    s = o.spins                                           # [z][y][x]
+    nT = -(-L // size)
+    u = np.arange(size)
+    U, V, W = np.meshgrid(u, u, u, indexing="ij")         # as [z][y][x] local coordinates
+    solid = np.ones((size, size, size), dtype=bool)
+    a, b, c = U.copy(), V.copy(), W.copy()
+    for _ in range(k):
+        ones = (a % 3 == 1).astype(int) + (b % 3 == 1) + (c % 3 == 1)
+        solid &= ones < 2
+        a //= 3; b //= 3; c //= 3
+    pattern = np.where(solid, 1, -1).astype(np.int8)
+    signs = []
+    for Z in range(nT):
+        for Y in range(nT):
+            for X in range(nT):
+                blk = s[Z * size:(Z + 1) * size, Y * size:(Y + 1) * size, X * size:(X + 1) * size]
+                pat = pattern[:blk.shape[0], :blk.shape[1], :blk.shape[2]]
+                T = (Z * nT + Y) * nT + X
+                bit = (py_philox([T >> 7, k, 0, 3], [seed & MASK, seed >> 32])[(T >> 5) & 3] >> (T & 31)) & 1
+                assert np.array_equal(blk, pat if bit else -pat), (X, Y, Z)
+                signs.append(bit)
+    assert o.sweep_count == 0
+    if len(signs) >= 8:
+        assert 0 < sum(signs) < len(signs)
+
+
+def test_init_menger_k0_is_an_iid_start():
+    """k = 0: one site per sponge, i.e. an iid p = 1/2 configuration."""
+    L = 32
+    o = orc.Oracle(L, 5, init=False)
+    o.init_menger(0)
+    N = L ** 3
+    n_up, a = o.measure([1, 2, 5])
+    assert abs(n_up - N / 2) < 4 * np.sqrt(N) / 2
+    assert np.all(np.abs(a.astype(float) - N / 2) < 4 * np.sqrt(N) / 2)
+
+
+def test_init_menger_tile_signs_fair():
+    L, k = 96, 1                                           # 32^3 tiles
+    o = orc.Oracle(L, 123, init=False)
+    o.init_menger(k)
+    corner = o.spins[::3, ::3, ::3]                        # (0,0,0) of every tile is solid
+    n = corner.size
+    assert abs((corner == 1).sum() - n / 2) < 4 * np.sqrt(n) / 2
+    # magnetisation of a sponge start: |m| per tile = (20 - 7)/27
+    tiles = o.spins.reshape(32, 3, 32, 3, 32, 3).sum(axis=(1, 3, 5))
+    assert set(np.unique(tiles)) <= {13, -13}
