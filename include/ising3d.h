@@ -79,6 +79,10 @@ extern "C" {
 #define ISING3D_VARIANT_RESIDENT 4  /* lattice resident in the shared memory of a thread-block
                                        cluster, all sweeps of a call in one launch (L in 64..256) */
 
+/* update order inside a sweep (ising3d_set_cycle) */
+#define ISING3D_CYCLE_01    0   /* colour 0 then colour 1, every sweep (main text) */
+#define ISING3D_CYCLE_MIXED 1   /* first colour drawn per sweep (Supp. I.B PAPER.md:258, D10)    */
+
 typedef struct ising3d ising3d_t;   /* opaque */
 
 /*
@@ -132,6 +136,31 @@ int ising3d_init_batch_with_buffer(ising3d_t **h, int L, int n_rep, const uint64
 
 /* Re-generate the T = infinity start (same seeds) and reset sweep to 0. Async. */
 int ising3d_reset(ising3d_t *h);
+
+/*
+ * Menger-sponge start (Fig. 4; reading D11): "The starting
+ * configuration of dimensions L^3 is created by repeating sponges of k-th iteration of size
+ * (3^k)^3.  For each sponge we pick uniformly at random whether the Menger structure is
+ * represented by up or down spins."  Tiles start at the origin, the last tile in each
+ * direction is cut at L; a site with local coordinates (u,v,w) is in the sponge iff at no
+ * ternary digit position two or more of u,v,w have digit 1; tile T = (Z*nT + Y)*nT + X,
+ * nT = ceil(L/3^k), takes its sign from bit (T & 127) of Philox(key = the replica's seed,
+ * counter = (T >> 7, k, 0, 3)): sponge sites +1 if the bit is 1, holes the opposite sign.
+ * k = 0 is an iid p = 1/2 start.  Replaces the state of every replica, sets sweep to 0.
+ * Asynchronous.  EINVAL unless 0 <= k <= 7 and 3^k <= L.
+ */
+int ising3d_init_menger(ising3d_t *h, int k);
+
+/*
+ * Choose the order of the two half-sweeps (ISING3D_CYCLE_*).  01 cycle (default): colour 0
+ * then colour 1 (D7).  Mixed cycle (Supp. I.B PAPER.md:258: "choosing at random
+ * which sublattice to update first ... still every spin is proposed to flip exactly once per
+ * sweep"; reading D10): in sweep t the replica with seed s updates first the colour given by
+ * bit 0 of word 0 of Philox(key = s, counter = (0, t, 0, 2)); the tie bits keep counter
+ * (q, t, c, 0) with c the colour being updated.  Takes effect from the next sweep.
+ * EINVAL for an unknown value or with ISING3D_VARIANT_FUSED (01 cycle only).
+ */
+int ising3d_set_cycle(ising3d_t *h, int cycle);
 
 /* Use `cuda_stream` (a cudaStream_t owned by the caller) for all later work. */
 int ising3d_set_stream(ising3d_t *h, void *cuda_stream);

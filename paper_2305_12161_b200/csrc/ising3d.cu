@@ -56,6 +56,7 @@ struct ising3d {
     uint64_t *d_seeds = nullptr;
     unsigned long long *d_counts = nullptr;
     int variant = ISING3D_VARIANT_AUTO;
+    int cycle = ISING3D_CYCLE_01;
     uint64_t launches = 0;
     int sm_count = 148;
     mutable ising::ResidentPlan res_plan = {0, 0};
@@ -93,7 +94,8 @@ struct ising3d {
     bool use_fused() const
     {
         return variant == ISING3D_VARIANT_FUSED ||
-               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok() && !resident_ok());
+               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok() && !resident_ok() &&
+                cycle == ISING3D_CYCLE_01);
     }
 };
 
@@ -188,12 +190,13 @@ int sweep_generic(ising3d *h, uint64_t n)
 {
     const size_t groups = h->words_per_replica() / 8;   // per colour
     dim3 grid((unsigned)((groups + 255) / 256), (unsigned)h->n_rep);
+    const int mixed = h->cycle == ISING3D_CYCLE_MIXED;
     for (uint64_t i = 0; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
         ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
-                                                                     h->L, t, 0);
+                                                                     h->L, t, 0, mixed);
         ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
-                                                                     h->L, t, 1);
+                                                                     h->L, t, 1, mixed);
     }
     h->launches += 2 * n;
     CUDA_TRY(cudaGetLastError());
@@ -203,7 +206,8 @@ int sweep_generic(ising3d *h, uint64_t n)
 int sweep_resident(ising3d *h, uint64_t n)
 {
     cudaError_t e = ising::launch_resident(h->state[h->cur], h->d_seeds, h->L, h->n_rep, h->res_plan,
-                                           (uint32_t)h->sweep, (uint32_t)n, h->stream);
+                                           (uint32_t)h->sweep, (uint32_t)n,
+                                           h->cycle == ISING3D_CYCLE_MIXED, h->stream);
     if (e != cudaSuccess)
         return fail(ISING3D_ECUDA, std::string("resident sweep launch: ") + cudaGetErrorString(e));
     h->launches += 1;
@@ -215,9 +219,11 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
     const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
     for (uint64_t i = 0; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
+        // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
+        const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(h->seeds[0], t) : 0;
         cudaError_t e =
             gen2 ? ising::launch_fused2_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t,
-                                              h->seeds[0], h->sm_count, h->stream)
+                                              h->seeds[0], first, h->sm_count, h->stream)
                  : ising::launch_fused_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t, keys,
                                              h->sm_count, h->stream);
         if (e != cudaSuccess)
@@ -303,11 +309,40 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream)
     return ISING3D_OK;
 }
 
+int ising3d_set_cycle(ising3d_t *h, int cycle)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (cycle != ISING3D_CYCLE_01 && cycle != ISING3D_CYCLE_MIXED)
+        return fail(ISING3D_EINVAL, "unknown cycle");
+    if (cycle == ISING3D_CYCLE_MIXED && h->variant == ISING3D_VARIANT_FUSED)
+        return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
+    h->cycle = cycle;
+    return ISING3D_OK;
+}
+
+int ising3d_init_menger(ising3d_t *h, int k)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    int size = 1;
+    for (int i = 0; i < k && size <= 4096; ++i) size *= 3;
+    if (k < 0 || k > 7 || size > h->L)
+        return fail(ISING3D_EINVAL, "Menger iteration k must satisfy 0 <= k and 3^k <= L");
+    const size_t words = h->words_per_replica();
+    dim3 grid((unsigned)((words + 255) / 256), (unsigned)h->n_rep);
+    ising::init_menger_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds, h->L, k, size);
+    h->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    h->sweep = 0;
+    return ISING3D_OK;
+}
+
 int ising3d_set_variant(ising3d_t *h, int variant)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_RESIDENT)
         return fail(ISING3D_EINVAL, "unknown variant");
+    if (variant == ISING3D_VARIANT_FUSED && h->cycle == ISING3D_CYCLE_MIXED)
+        return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
         return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())

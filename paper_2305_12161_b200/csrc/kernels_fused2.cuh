@@ -42,7 +42,10 @@ struct SweepConsts {
     uint32_t k1[10];
 };
 
-inline SweepConsts make_sweep_consts(uint64_t seed, uint32_t t)
+// `first` = colour updated first in this sweep (0 for the 01 cycle; drawn per sweep in the mixed
+// cycle, D10).  The kernel's "black" role is colour `first`, its "white" role colour 1-first;
+// c1[role] carries the role's colour into the Philox counter.
+inline SweepConsts make_sweep_consts(uint64_t seed, uint32_t t, int first = 0)
 {
     SweepConsts s;
     const PhiloxKeys k = make_philox_keys(seed);
@@ -52,8 +55,8 @@ inline SweepConsts make_sweep_consts(uint64_t seed, uint32_t t)
     }
     s.a0 = t ^ k.k0[0];
     s.r0k1 = k.k1[0];
-    s.c1[0] = 0u ^ k.k0[1];
-    s.c1[1] = kPhiloxM1 ^ k.k0[1];
+    s.c1[0] = (first ? kPhiloxM1 : 0u) ^ k.k0[1];
+    s.c1[1] = (first ? 0u : kPhiloxM1) ^ k.k0[1];
     const uint64_t p0 = (uint64_t)kPhiloxM0 * s.a0;
     s.d1 = (uint32_t)(p0 >> 32) ^ k.k1[1];
     s.e2 = (uint32_t)p0 ^ k.k1[2];
@@ -203,7 +206,8 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
 template <int R4, int NT>
 __global__ void __launch_bounds__(NT, 2)
 fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, const int L,
-                    const int RPT, const int nzc, const __grid_constant__ SweepConsts keys)
+                    const int RPT, const int nzc, const int first,
+                    const __grid_constant__ SweepConsts keys)
 {
     constexpr int TY = 2 * NT / R4;    // rows in the tile (incl. 2+2 halo rows)
     constexpr int PLANE = TY * R4;     // uint4 per plane tile
@@ -220,8 +224,11 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     const int x4 = tid & (R4 - 1), p = tid / R4;     // group column, row pair
     const int ry = 2 * p;                            // even tile row of this thread
     const int jt = blockIdx.x, zc = blockIdx.y;
-    const int zs = ((int)((long long)L * zc / nzc)) | 1;
-    const int ze = zc + 1 == nzc ? (L | 1) : (((int)((long long)L * (zc + 1) / nzc)) | 1);
+    // chunk borders have the parity of 1-first, so that (z0 + first) is even for z0 = zs-3 and
+    // the in-row direction o = (y + z + colour) & 1 of the even tile row at step k is k & 1
+    const int b0 = (int)((long long)L * zc / nzc), b1 = zc + 1 == nzc ? L : (int)((long long)L * (zc + 1) / nzc);
+    const int zs = first ? (b0 & ~1) : (b0 | 1);
+    const int ze = first ? (b1 & ~1) : (b1 | 1);
     const int nz = ze - zs;
     const int K = nz + 4;                  // steps: 2 window fills, nz+1 black, nz white
     int ybase = jt * RPT - 2;
@@ -235,8 +242,9 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     c.Bst = Bst;
     c.nb = nb;
     c.bars = bars;
-    c.dstB = dst;
-    c.dstW = dst + G;
+    const uint4 *srcB = src + (first ? G : 0), *srcW = src + (first ? 0 : G);
+    c.dstB = dst + (first ? G : 0);
+    c.dstW = dst + (first ? 0 : G);
     c.si0 = ry * R4 + x4;
     c.si_ym = ry > 0 ? c.si0 - R4 : c.si0;
     c.si_yp = ry + 2 < TY ? c.si0 + 2 * R4 : c.si0;
@@ -262,8 +270,8 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     const uint32_t bytes1 = (uint32_t)n1 * R4 * 16u, bytes2 = (uint32_t)(TY - n1) * R4 * 16u;
     const size_t plane_u4 = (size_t)L * R4;
     int pzw = ((zs - 2) % L + L) % L, pzb = ((zs - 3) % L + L) % L, pk = 0;
-    const uint4 *pgw = src + G + (size_t)pzw * plane_u4;
-    const uint4 *pgb = src + (size_t)pzb * plane_u4;
+    const uint4 *pgw = srcW + (size_t)pzw * plane_u4;
+    const uint4 *pgb = srcB + (size_t)pzb * plane_u4;
     auto issue_next = [&]() {
         const int s = pk & (S - 1);
         const uint32_t bar = smem_u32(&bars[s]);
@@ -277,8 +285,8 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
         ++pk;
         pgw += plane_u4;
         pgb += plane_u4;
-        if (++pzw == L) { pzw = 0; pgw = src + G; }
-        if (++pzb == L) { pzb = 0; pgb = src; }
+        if (++pzw == L) { pzw = 0; pgw = srcW; }
+        if (++pzb == L) { pzb = 0; pgb = srcB; }
     };
     if (tid == 0)
         for (int k = 0; k < D && k < K; ++k) issue_next();
@@ -321,7 +329,7 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
 inline bool fused2_supported(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096; }
 
 template <int R4, int NT>
-inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L,
+inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first,
                                    const SweepConsts &keys, int sm_count, cudaStream_t stream)
 {
     constexpr int TY = 2 * NT / R4;
@@ -349,19 +357,19 @@ inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L,
     }
     dim3 grid((unsigned)nty, (unsigned)nzc);
     fused2_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(
-        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, RPT, nzc, keys);
+        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, RPT, nzc, first, keys);
     return cudaGetLastError();
 }
 
 inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
-                                       uint64_t seed, int sm_count, cudaStream_t stream)
+                                       uint64_t seed, int first, int sm_count, cudaStream_t stream)
 {
-    const SweepConsts keys = make_sweep_consts(seed, t);
+    const SweepConsts keys = make_sweep_consts(seed, t, first);
     switch (L) {
-        case 512:  return launch_fused2_t<2, 128>(src, dst, L, keys, sm_count, stream);
-        case 1024: return launch_fused2_t<4, 256>(src, dst, L, keys, sm_count, stream);
-        case 2048: return launch_fused2_t<8, 256>(src, dst, L, keys, sm_count, stream);
-        case 4096: return launch_fused2_t<16, 256>(src, dst, L, keys, sm_count, stream);
+        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, keys, sm_count, stream);
+        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, keys, sm_count, stream);
+        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, keys, sm_count, stream);
+        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, keys, sm_count, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

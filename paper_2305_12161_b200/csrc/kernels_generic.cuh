@@ -25,18 +25,70 @@ init_spins_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ see
     reinterpret_cast<uint4 *>(state)[(size_t)rep * 2 * groups_per_colour + g] = v;
 }
 
+// `phase` = 0 / 1: first / second half-sweep of sweep t.  01 cycle (mixed = 0): colour = phase.
+// Mixed cycle (mixed = 1, D10): colour = phase ^ first_colour(seed of the replica, t).
+// Menger-sponge start (D11): the lattice is tiled from the origin by sponges of
+// iteration k and edge size = 3^k (the last tile in each direction is cut at L); a site belongs
+// to the sponge iff at no ternary digit position two or more of its local coordinates have the
+// digit 1; tile T = (Z*nT + Y)*nT + X draws its sign from Philox(counter (T >> 7, k, 0, 3)) bit
+// T & 127; sponge sites take that sign, holes the opposite.  One thread per packed word.
+__global__ void __launch_bounds__(256)
+init_menger_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds, int L, int k,
+                   int size)
+{
+    const int WPR = L >> 6;
+    const size_t WPC = (size_t)L * L * WPR;
+    const size_t w = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= 2 * WPC) return;
+    const int rep = blockIdx.y;
+    const uint64_t seed = seeds[rep];
+    const int c = w >= WPC ? 1 : 0;
+    const size_t wc = w - (size_t)c * WPC;
+    const int wi = (int)(wc % WPR);
+    const size_t row = wc / WPR;
+    const int y = (int)(row % L), z = (int)(row / L);
+    const int o = (y + z + c) & 1;
+    const int nT = (L + size - 1) / size;
+    const int Y = y / size, Z = z / size, v = y - Y * size, ww = z - Z * size;
+    uint32_t out = 0, cached_group = 0xFFFFFFFFu;
+    uint4 rnd = make_uint4(0, 0, 0, 0);
+    for (int j = 0; j < 32; ++j) {
+        const int x = 2 * (32 * wi + j) + o;
+        const int X = x / size;
+        int a = x - X * size, b = v, d = ww;
+        bool solid = true;
+        for (int level = 0; level < k; ++level) {
+            const int ones = (a % 3 == 1) + (b % 3 == 1) + (d % 3 == 1);
+            if (ones >= 2) solid = false;
+            a /= 3; b /= 3; d /= 3;
+        }
+        const uint32_t T = (uint32_t)((Z * nT + Y) * nT + X);
+        if ((T >> 7) != cached_group) {
+            cached_group = T >> 7;
+            rnd = philox4x32_10(cached_group, (uint32_t)k, 0u, kTagMenger, (uint32_t)seed,
+                                (uint32_t)(seed >> 32));
+        }
+        const uint32_t word = ((T >> 5) & 3) == 0 ? rnd.x : ((T >> 5) & 3) == 1 ? rnd.y
+                            : ((T >> 5) & 3) == 2 ? rnd.z : rnd.w;
+        const uint32_t bit = (word >> (T & 31)) & 1u;
+        out |= (solid ? bit : bit ^ 1u) << j;
+    }
+    state[(size_t)rep * 2 * WPC + w] = out;
+}
+
 __global__ void __launch_bounds__(256)
 halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
-                         int L, uint32_t t, int c)
+                         int L, uint32_t t, int phase, int mixed)
 {
     const int WPR = L >> 6;                                   // words per row
     const size_t WPC = (size_t)L * L * WPR;                   // words per colour
     const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= WPC / 4) return;
     const int rep = blockIdx.y;
+    const uint64_t seed = seeds[rep];
+    const int c = mixed ? phase ^ first_colour(seed, t) : phase;
     uint32_t *own = state + (size_t)rep * 2 * WPC + (size_t)c * WPC;
     const uint32_t *oth = state + (size_t)rep * 2 * WPC + (size_t)(1 - c) * WPC;
-    const uint64_t seed = seeds[rep];
     const uint4 rnd = philox4x32_10((uint32_t)g, t, (uint32_t)c, 0u, (uint32_t)seed,
                                     (uint32_t)(seed >> 32));
     const uint32_t rho[4] = {rnd.x, rnd.y, rnd.z, rnd.w};

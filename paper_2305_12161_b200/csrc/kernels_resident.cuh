@@ -68,7 +68,7 @@ __device__ __forceinline__ uint4 res_update_group(const uint4 own, const uint4 p
 template <int WPR>
 __global__ void __launch_bounds__(kResThreads, 1)
 resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
-                      const uint32_t t0, const uint32_t n_sweeps)
+                      const uint32_t t0, const uint32_t n_sweeps, const int mixed)
 {
     constexpr int L = 64 * WPR;
     constexpr int GPP = L * WPR / 4;              // 128-bit groups per plane
@@ -87,7 +87,6 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
     uint4 *gstate = reinterpret_cast<uint4 *>(state) + (size_t)rep * 2 * GPC;
 
     // slot s of colour c = plane z0 - 1 + s  (s = 0 lower halo, 1..PZ own, PZ + 1 upper halo)
-    uint4 *col_base[2] = {res_smem, res_smem + (size_t)(PZ + 2) * GPP};
 
     // ---- load: own planes and halos of both colours from HBM ----
     for (int idx = tid; idx < 2 * (PZ + 2) * GPP; idx += kResThreads) {
@@ -119,22 +118,23 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
     const int g_prev = g == 0 ? GPP - 1 : g - 1, g_next = g == GPP - 1 ? 0 : g + 1;
     const int y0 = 4 * g / WPR;                   // first row of the group
 
-    // halo slots of the neighbouring CTAs (distributed shared memory)
+    // halo slots of the neighbouring CTAs (distributed shared memory); colour c of a CTA starts
+    // at res_smem + c * CSTRIDE
+    const size_t CSTRIDE = (size_t)(PZ + 2) * GPP;
     const int rank_dn = rank == 0 ? CS - 1 : rank - 1, rank_up = rank == CS - 1 ? 0 : rank + 1;
-    uint4 *peer_dn[2], *peer_up[2];
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-        peer_dn[c] = cluster.map_shared_rank(col_base[c], rank_dn);   // its slot PZ+1 <- my plane 0
-        peer_up[c] = cluster.map_shared_rank(col_base[c], rank_up);   // its slot 0    <- my plane PZ-1
-    }
+    uint4 *peer_dn = cluster.map_shared_rank(res_smem, rank_dn);   // its slot PZ+1 <- my plane 0
+    uint4 *peer_up = cluster.map_shared_rank(res_smem, rank_up);   // its slot 0    <- my plane PZ-1
     cluster.sync();                               // everybody loaded; peers' smem exists
 
     for (uint32_t it = 0; it < n_sweeps; ++it) {
         const uint32_t t = t0 + it;
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-            uint4 *own = col_base[c];
-            const uint4 *oth = col_base[1 - c];
+        // 01 cycle: colour 0 first (D7); mixed cycle: the first colour is drawn per sweep (D10)
+        const int first = mixed ? first_colour(seed, t) : 0;
+#pragma unroll 1
+        for (int phase = 0; phase < 2; ++phase) {
+            const int c = phase ^ first;
+            uint4 *own = res_smem + (size_t)c * CSTRIDE;
+            const uint4 *oth = res_smem + (size_t)(1 - c) * CSTRIDE;
             if (active) {
                 for (int zl = pl; zl < PZ; zl += PPI) {
                     const int z = z0 + zl;
@@ -143,12 +143,12 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
                     const uint4 zm = pz[g - GPP], zp = pz[g + GPP];
                     const uint4 o4 = own[(size_t)(zl + 1) * GPP + g];
                     const uint32_t q = (uint32_t)z * GPP + g;
-                    const uint4 rho = philox4x32_10(q, t, (uint32_t)c, 0u, keys);
+                    const uint4 rho = philox4x32_10(q, t, (uint32_t)c, kTagTie, keys);
                     const uint4 nw = res_update_group<WPR>(o4, prv, sam, nxt, zm, zp, rho,
                                                            (y0 + z + c) & 1);
                     own[(size_t)(zl + 1) * GPP + g] = nw;
-                    if (zl == 0) peer_dn[c][(size_t)(PZ + 1) * GPP + g] = nw;
-                    if (zl == PZ - 1) peer_up[c][g] = nw;
+                    if (zl == 0) peer_dn[(size_t)c * CSTRIDE + (size_t)(PZ + 1) * GPP + g] = nw;
+                    if (zl == PZ - 1) peer_up[(size_t)c * CSTRIDE + g] = nw;
                 }
             }
             cluster.sync();
@@ -234,7 +234,7 @@ inline ResidentPlan resident_plan(int L, int n_rep, int sm_count)
 template <int WPR>
 inline cudaError_t launch_resident_t(uint32_t *state, const uint64_t *d_seeds, int n_rep,
                                      const ResidentPlan &plan, uint32_t t0, uint32_t n_sweeps,
-                                     cudaStream_t stream)
+                                     int mixed, cudaStream_t stream)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)plan.cs, (unsigned)n_rep);
@@ -248,17 +248,17 @@ inline cudaError_t launch_resident_t(uint32_t *state, const uint64_t *d_seeds, i
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, resident_sweep_kernel<WPR>, state, d_seeds, t0, n_sweeps);
+    return cudaLaunchKernelEx(&cfg, resident_sweep_kernel<WPR>, state, d_seeds, t0, n_sweeps, mixed);
 }
 
 inline cudaError_t launch_resident(uint32_t *state, const uint64_t *d_seeds, int L, int n_rep,
                                    const ResidentPlan &plan, uint32_t t0, uint32_t n_sweeps,
-                                   cudaStream_t stream)
+                                   int mixed, cudaStream_t stream)
 {
     switch (L) {
-        case 64:  return launch_resident_t<1>(state, d_seeds, n_rep, plan, t0, n_sweeps, stream);
-        case 128: return launch_resident_t<2>(state, d_seeds, n_rep, plan, t0, n_sweeps, stream);
-        case 256: return launch_resident_t<4>(state, d_seeds, n_rep, plan, t0, n_sweeps, stream);
+        case 64:  return launch_resident_t<1>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
+        case 128: return launch_resident_t<2>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
+        case 256: return launch_resident_t<4>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
         default:  return cudaErrorInvalidValue;
     }
 }

@@ -54,9 +54,10 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
-// key schedule in registers (batched replicas: the seed is per block)
-__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               uint32_t k0, uint32_t k1)
+// key schedule in registers (batched replicas: the seed is per block); also callable on the
+// host, where the launch layer draws the per-sweep colour order of the mixed cycle (D10)
+__host__ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2,
+                                                        uint32_t c3, uint32_t k0, uint32_t k1)
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -72,6 +73,18 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
         k1 += kPhiloxW1;
     }
     return make_uint4(c0, c1, c2, c3);
+}
+
+// Counter tags (domain separation, D5/D10/D11)
+constexpr uint32_t kTagTie = 0u;       // tie bits of sweep t:          counter (q, t, colour, 0)
+constexpr uint32_t kTagInit = 1u;      // T = infinity start:           counter (q, 0, colour, 1)
+constexpr uint32_t kTagOrder = 2u;     // mixed cycle, first colour:    counter (0, t, 0, 2), word 0 bit 0
+constexpr uint32_t kTagMenger = 3u;    // Menger start, tile sign bits: counter (T >> 7, k, 0, 3)
+
+// Mixed cycle (Supp. I.B PAPER.md:258, D10): the colour updated first in sweep t.
+__host__ __device__ __forceinline__ int first_colour(uint64_t seed, uint32_t t)
+{
+    return (int)(philox4x32_10(0u, t, 0u, kTagOrder, (uint32_t)seed, (uint32_t)(seed >> 32)).x & 1u);
 }
 
 // ---------------------------------------------------------------------------

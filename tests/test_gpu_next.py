@@ -1,0 +1,163 @@
+"""GPU parity of the SURVEY.md 8(f) rows built so far, through the C ABI, against the oracle:
+mixed cycle (f-2, Supp. I.B PAPER.md:258, D10) and Menger-sponge start (f-3, D11).
+Bit-exact states and counts; C(r), ell within 1e-12 relative."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2305_12161_b200 import inputs  # noqa: E402
+from test_gpu_parity import check_measure, VARIANTS, _sample_sites, _bits_at  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2305_12161_b200 import build, binding
+    build.build()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    oracle.build()
+    return oracle
+
+
+# ------------------------------------------------------------------ f-2: mixed cycle
+@pytest.mark.parametrize("L,seed,variant,cps", [
+    (64, 1, "resident", [1, 2, 5, 20]), (64, 5, "generic", [1, 7]), (128, 7, "resident", [3, 12]),
+    (192, 8, "generic", [1, 4]), (256, 2, "resident", [2, 9]), (256, 2, "generic", [3]),
+    (512, 11, "fused2", [1, 2, 6]), (1024, 3, "fused2", [1, 3])])
+def test_mixed_cycle_against_oracle(B, orc, L, seed, variant, cps):
+    sim = B.Ising3D(L, [seed], variant=VARIANTS(B)[variant])
+    sim.set_cycle(B.CYCLE_MIXED)
+    assert sim.variant_name == variant
+    ref = orc.Oracle(L, seed)
+    t = 0
+    for cp in cps:
+        sim.sweep(cp - t)
+        ref.sweep_mixed(cp - t)
+        t = cp
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+    if L <= 512:
+        check_measure(sim.measure(), ref.measure_full())
+    # the orders drawn so far contained both colours (else the test proves nothing)
+    assert {orc.first_colour(seed, s) for s in range(cps[-1])} == {0, 1} or cps[-1] < 3
+    sim.free()
+
+
+def test_mixed_cycle_batch_draws_an_order_per_replica(B, orc):
+    L, seeds = 128, [100, 101, 102, 103, 131, 163]
+    batch = B.Ising3D(L, seeds)
+    batch.set_cycle(B.CYCLE_MIXED)
+    assert batch.variant_name == "resident"
+    refs = [orc.Oracle(L, s) for s in seeds]
+    assert len({tuple(orc.first_colour(s, t) for t in range(6)) for s in seeds}) > 1
+    for n in (1, 5):
+        batch.sweep(n)
+        st = batch.get_state().reshape(len(seeds), -1)
+        for i, ref in enumerate(refs):
+            ref.sweep_mixed(n)
+            assert np.array_equal(st[i], ref.export_words())
+    batch.free()
+
+
+def test_mixed_cycle_neel_closed_form_on_gpu(B, orc):
+    """One mixed sweep from the Neel state orders the lattice with the value of the colour
+    updated second (closed form, see tests/test_oracle_next.py): reads out the order used."""
+    for L, variant in ((64, "resident"), (512, "fused2"), (192, "generic")):
+        sim = B.Ising3D(L, [11], variant=VARIANTS(B)[variant])
+        sim.set_cycle(B.CYCLE_MIXED)
+        words = inputs.pack_spins(inputs.neel(L))
+        for t in range(6):
+            sim.set_state(words, t)
+            sim.sweep(1)
+            first = orc.first_colour(11, t)
+            want = np.full(L ** 3 // 32, 0xFFFFFFFF if first else 0, dtype=np.uint32)
+            assert np.array_equal(sim.get_state(), want)
+        sim.free()
+
+
+def test_mixed_cycle_full_size_sampled(B, orc):
+    """L = 2048 in the bench launch configuration, mixed cycle: fused2 == generic word for word
+    over sweeps whose drawn orders differ."""
+    L, seed = 2048, 4
+    a = B.Ising3D(L, [seed])
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_GENERIC)
+    a.set_cycle(B.CYCLE_MIXED)
+    b.set_cycle(B.CYCLE_MIXED)
+    assert a.variant_name == "fused2"
+    assert {orc.first_colour(seed, t) for t in range(4)} == {0, 1}
+    for n in (1, 3):
+        a.sweep(n)
+        b.sweep(n)
+        assert np.array_equal(a.get_state(), b.get_state())
+    a.free()
+    b.free()
+
+
+def test_cycle_errors(B):
+    sim = B.Ising3D(256, [1], variant=B.VARIANT_FUSED)
+    with pytest.raises(B.Ising3DError):
+        sim.set_cycle(B.CYCLE_MIXED)
+    with pytest.raises(B.Ising3DError):
+        sim.set_cycle(7)
+    sim.free()
+
+
+# ------------------------------------------------------------------ f-3: Menger sponge
+@pytest.mark.parametrize("L,k,seed", [(64, 0, 3), (64, 1, 3), (64, 2, 4), (64, 3, 5), (128, 3, 6),
+                                      (192, 2, 7), (256, 4, 8)])
+def test_menger_start_and_quench(B, orc, L, k, seed):
+    sim = B.Ising3D(L, [seed])
+    sim.sweep(2)
+    sim.init_menger(k)
+    assert sim.sweep_count == 0
+    ref = orc.Oracle(L, seed, init=False)
+    ref.init_menger(k)
+    assert np.array_equal(sim.get_state(), ref.export_words()), "Menger start differs"
+    for n in (1, 4):
+        sim.sweep(n)
+        ref.sweep(n)
+        assert np.array_equal(sim.get_state(), ref.export_words())
+    check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+
+
+def test_menger_batch_and_errors(B, orc):
+    L, seeds = 128, [100, 101, 163]
+    batch = B.Ising3D(L, seeds)
+    batch.init_menger(2)
+    st = batch.get_state().reshape(3, -1)
+    for i, s in enumerate(seeds):
+        ref = orc.Oracle(L, s, init=False)
+        ref.init_menger(2)
+        assert np.array_equal(st[i], ref.export_words())
+    assert not np.array_equal(st[0], st[1])
+    with pytest.raises(B.Ising3DError):
+        batch.init_menger(5)          # 3^5 = 243 > L
+    with pytest.raises(B.Ising3DError):
+        batch.init_menger(-1)
+    batch.free()
+
+
+def test_menger_full_size_structure(B, orc):
+    """L = 512, k = 3 (the paper's Fig. 4(c) size): sampled sites against the oracle's
+    menger_solid and tile signs read off the solid corner site of each tile."""
+    L, k, seed = 512, 3, 9
+    sim = B.Ising3D(L, [seed])
+    sim.init_menger(k)
+    words = sim.get_state()
+    rng = np.random.Generator(np.random.PCG64(1))
+    xyz = rng.integers(0, L, size=(4000, 3)).astype(np.int32)
+    got = _bits_at(words, L, xyz)
+    corner = (xyz // 27) * 27
+    sign = _bits_at(words, L, corner.astype(np.int32))      # local (0,0,0) is always solid
+    solid = np.array([orc.menger_solid(int(x % 27), int(y % 27), int(z % 27), k) for x, y, z in xyz])
+    assert np.array_equal(got, np.where(solid == 1, sign, -sign))
+    m = sim.measure()
+    assert 0 < int(m["n_up"][0]) < L ** 3
+    sim.free()
