@@ -42,6 +42,7 @@ def parse():
     ap.add_argument("--L", type=int, default=2048)
     ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (throughput window)")
     ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2"])
+    ap.add_argument("--ref-L", type=int, default=512, help="--impl reference: lattice size of the CPU sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-measure", action="store_true", help="step = reset + sweeps only")
@@ -130,7 +131,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from oracle import oracle as orc
-    L, n_sw, seed = 512, 20, 4
+    L, n_sw, seed = args.ref_L, 20, 4
     sample = ("L=%d (config-5 start rule: iid p=1/2 from seed %d), sweeps 0..%d per step; "
               "the oracle cannot hold 1000 sweeps of L=2048 in minutes" % (L, seed, n_sw - 1))
     for _ in range(args.warmup):
@@ -153,6 +154,30 @@ def run_reference(args):
     }
     print(json.dumps(line))
     return 0
+
+
+# ----------------------------------------------------------------------------- replicas only
+# The path does not shard (one lattice per GPU): N ranks = N independent lattices,
+# no data-path collective.  What the ranks share is the timing protocol below (covered on CPU by
+# the world_size-2 gloo test in tests/test_bench_host.py).
+def rank_seed(rank: int) -> int:
+    """Config 5 uses seed 4; replica r of an N-GPU run uses seed 4 + r."""
+    return 4 + rank
+
+
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Device time of the slowest rank (the contract's max over ranks)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world: int, n_sites: int, sweeps: int, steps: int, ms_max: float) -> float:
+    """site-updates/ns of the whole job: every rank did n_sites * sweeps * steps proposals."""
+    return world * n_sites * sweeps * steps / (ms_max * 1e6)
 
 
 # ----------------------------------------------------------------------------- ours
@@ -203,7 +228,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     L, S = args.L, args.sweeps
-    seed = 4 + rank                                   # config 5: seed 4 (replica r: 4 + r)
+    seed = rank_seed(rank)
     variant = {"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
                "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2}[args.variant]
     sim = binding.Ising3D(L, [seed], variant=variant)
@@ -244,11 +269,8 @@ def run_ours(args):
     init_ms = sum(t[0].elapsed_time(t[1]) for t in timers) / args.steps
     sweep_ms = sum(t[1].elapsed_time(t[2]) for t in timers) / args.steps
     meas_ms = sum(t[2].elapsed_time(t[3]) for t in timers) / args.steps
-    tmax = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tmax.item())
-    value = world * N * S * args.steps / (total_ms_max * 1e6)
+    total_ms_max = max_over_ranks(total_ms, world, "cuda")
+    value = whole_job_rate(world, N, S, args.steps, total_ms_max)
 
     # ---------------- end to end through the C ABI with HOST buffers ----------------
     e2e = None
@@ -273,12 +295,10 @@ def run_ours(args):
             r = sim.measure()                                   # D2H of the step's result
         t1.record()
         barrier()
-        ems = torch.tensor([t0.elapsed_time(t1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(ems, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * N * S * k_e2e / (float(ems.item()) * 1e6), "unit": UNIT,
+        ems = max_over_ranks(t0.elapsed_time(t1), world, "cuda")
+        e2e = {"value": whole_job_rate(world, N, S, k_e2e, ems), "unit": UNIT,
                "h2d_bytes_per_step": n_words * 4, "d2h_bytes_per_step": d2h_bytes,
-               "ms_per_step": float(ems.item()) / k_e2e,
+               "ms_per_step": ems / k_e2e,
                "note": "set_state(pinned host, 1 GiB at L=2048) + sweep + measure(host counts) per step"}
 
     if rank != 0:
