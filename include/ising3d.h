@@ -79,6 +79,11 @@ extern "C" {
 #define ISING3D_VARIANT_RESIDENT 4  /* lattice resident in the shared memory of a thread-block
                                        cluster, all sweeps of a call in one launch (L in 64..256) */
 
+/* measurement kernels (ising3d_set_measure_variant) */
+#define ISING3D_MEASURE_AUTO     0  /* tensor where the shape allows (L % 512 == 0), else popcount */
+#define ISING3D_MEASURE_POPCOUNT 1  /* XOR + carry-save popcount over line words, any L             */
+#define ISING3D_MEASURE_TENSOR   2  /* pair counts as diagonals of a Gram matrix: tcgen05 int8 MMA  */
+
 /* update order inside a sweep (ising3d_set_cycle) */
 #define ISING3D_CYCLE_01    0   /* colour 0 then colour 1, every sweep (main text) */
 #define ISING3D_CYCLE_MIXED 1   /* first colour drawn per sweep (Supp. I.B PAPER.md:258, D10)    */
@@ -136,6 +141,10 @@ int ising3d_init_batch_with_buffer(ising3d_t **h, int L, int n_rep, const uint64
 
 /* Re-generate the T = infinity start (same seeds) and reset sweep to 0. Async. */
 int ising3d_reset(ising3d_t *h);
+
+/* Choose the kernels behind the A_mu(r) counts of ising3d_measure (ISING3D_MEASURE_*).  Both
+ * give the same integers (D8).  EINVAL if the shape does not support the requested variant. */
+int ising3d_set_measure_variant(ising3d_t *h, int variant);
 
 /*
  * Menger-sponge start (Fig. 4; reading D11): "The starting
@@ -204,6 +213,8 @@ uint64_t ising3d_sweep_count(const ising3d_t *h);
 uint64_t ising3d_launch_count(const ising3d_t *h);
 /* name of the sweep kernel the handle currently dispatches to ("generic", "fused", ...) */
 const char *ising3d_variant_name(const ising3d_t *h);
+/* "tensor" or "popcount": the measurement kernels the handle dispatches to */
+const char *ising3d_measure_variant_name(const ising3d_t *h);
 /* CTAs per thread-block cluster (= SMs per lattice) of the resident kernel; 0 if another
  * kernel is dispatched. */
 int ising3d_cluster_size(const ising3d_t *h);

@@ -18,11 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libising3d.so")
 
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 CYCLE_01, CYCLE_MIXED = 0, 1
+MEASURE_AUTO, MEASURE_POPCOUNT, MEASURE_TENSOR = 0, 1, 2
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT = 0, 1, 2, 3, 4
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
-    "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_init_menger",
+    "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_init_menger", "ising3d_set_measure_variant",
+    "ising3d_measure_variant_name",
     "ising3d_sweep", "ising3d_measure", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
     "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size", "ising3d_sync",
@@ -67,6 +69,8 @@ def load():
         "ising3d_set_stream": (C.c_int, [vp, vp]),
         "ising3d_set_variant": (C.c_int, [vp, C.c_int]),
         "ising3d_set_cycle": (C.c_int, [vp, C.c_int]),
+        "ising3d_set_measure_variant": (C.c_int, [vp, C.c_int]),
+        "ising3d_measure_variant_name": (C.c_char_p, [vp]),
         "ising3d_init_menger": (C.c_int, [vp, C.c_int]),
         "ising3d_sweep": (C.c_int, [vp, u64]),
         "ising3d_measure": (C.c_int, [vp, C.POINTER(MeasT)]),
@@ -166,6 +170,13 @@ class Ising3D:
 
     def set_variant(self, variant: int):
         _check(self._l.ising3d_set_variant(self._h, variant))
+
+    def set_measure_variant(self, variant: int):
+        _check(self._l.ising3d_set_measure_variant(self._h, variant))
+
+    @property
+    def measure_variant_name(self) -> str:
+        return self._l.ising3d_measure_variant_name(self._h).decode()
 
     def set_cycle(self, cycle: int):
         _check(self._l.ising3d_set_cycle(self._h, cycle))

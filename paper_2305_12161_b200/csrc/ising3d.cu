@@ -16,6 +16,7 @@
 #include "kernels_fused.cuh"
 #include "kernels_fused2.cuh"
 #include "kernels_generic.cuh"
+#include "kernels_gram.cuh"
 #include "kernels_measure.cuh"
 #include "kernels_resident.cuh"
 #include "philox.cuh"
@@ -57,6 +58,9 @@ struct ising3d {
     unsigned long long *d_counts = nullptr;
     int variant = ISING3D_VARIANT_AUTO;
     int cycle = ISING3D_CYCLE_01;
+    int measure_variant = ISING3D_MEASURE_AUTO;
+    unsigned long long *d_gsum = nullptr;      // [n_rep][3][L/2+1] Gram diagonal sums
+    unsigned int *d_queue = nullptr;           // [3 n_rep] task counters of gram_kernel
     uint64_t launches = 0;
     int sm_count = 148;
     mutable ising::ResidentPlan res_plan = {0, 0};
@@ -67,6 +71,11 @@ struct ising3d {
     int counts_per_replica() const { return 1 + 3 * (L / 2 + 1); }
     bool fused_ok() const { return n_rep == 1 && ising::fused_supported(L); }
     bool fused2_ok() const { return n_rep == 1 && ising::fused2_supported(L); }
+    bool use_gram() const
+    {
+        return measure_variant == ISING3D_MEASURE_TENSOR ||
+               (measure_variant == ISING3D_MEASURE_AUTO && ising::gram_supported(L));
+    }
     bool resident_ok() const
     {
         if (!ising::resident_supported(L)) return false;
@@ -102,7 +111,7 @@ struct ising3d {
 namespace {
 
 struct Layout {
-    size_t state, seeds, counts, total;
+    size_t state, seeds, counts, gsum, queue, total;
 };
 
 Layout make_layout(int L, int n_rep)
@@ -111,7 +120,9 @@ Layout make_layout(int L, int n_rep)
     l.state = align_up((size_t)L * L * L / 8 * (size_t)n_rep, 256);
     l.seeds = align_up((size_t)n_rep * 8, 256);
     l.counts = align_up((size_t)n_rep * (1 + 3 * (L / 2 + 1)) * 8, 256);
-    l.total = 2 * l.state + l.seeds + l.counts;
+    l.gsum = align_up((size_t)n_rep * 3 * (L / 2 + 1) * 8, 256);
+    l.queue = align_up((size_t)n_rep * 3 * 4, 256);
+    l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue;
     return l;
 }
 
@@ -165,6 +176,8 @@ int create(ising3d_t **out, int L, int n_rep, const uint64_t *seeds, void *dev_b
         h->state[1] = (uint32_t *)(p + lay.state);
         h->d_seeds = (uint64_t *)(p + 2 * lay.state);
         h->d_counts = (unsigned long long *)(p + 2 * lay.state + lay.seeds);
+        h->d_gsum = (unsigned long long *)(p + 2 * lay.state + lay.seeds + lay.counts);
+        h->d_queue = (unsigned int *)(p + 2 * lay.state + lay.seeds + lay.counts + lay.gsum);
         int dev = 0;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
             (e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev)) !=
@@ -262,6 +275,49 @@ void postprocess(int L, uint64_t n_up, const uint64_t *antipar, double c_interce
     }
 }
 
+// A_mu(r) on the tensor cores (kernels_gram.cuh): per replica and axis, gather the line words
+// into the spare ping-pong buffer, run the Gram kernel, then A = 2 N_up - 2 Gsum.
+int measure_gram(ising3d *h)
+{
+    const int L = h->L, nr = L / 2 + 1, cpr = h->counts_per_replica();
+    static bool attr_set = false;
+    const size_t smem = ising::gram_smem_bytes(L);
+    const int NWB = L <= 2048 ? 8 : 4;
+    const size_t smem_x = (size_t)64 * NWB * (L / 32 + 1) * 4;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(ising::gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)ising::gram_smem_bytes(4096)));
+        CUDA_TRY(cudaFuncSetAttribute(ising::gather_lines_x_kernel,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024));
+        attr_set = true;
+    }
+    const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
+    CUDA_TRY(cudaMemsetAsync(h->d_gsum, 0, (size_t)h->n_rep * 3 * nr * 8, h->stream));
+    CUDA_TRY(cudaMemsetAsync(h->d_queue, 0, (size_t)h->n_rep * 3 * 4, h->stream));
+    const size_t wpr = h->words_per_replica();
+    const int WPR = L >> 6;
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        const uint32_t *st = h->state[h->cur] + (size_t)rep * wpr;
+        uint32_t *xw = h->state[1 - h->cur] + (size_t)rep * wpr;       // scratch: the other buffer
+        for (int ax = 0; ax < 3; ++ax) {
+            if (ax == 0)
+                ising::gather_lines_x_kernel<<<(unsigned)(L * (WPR / NWB)), 256, smem_x, h->stream>>>(st, xw, L, NWB);
+            else if (ax == 1)
+                ising::gather_lines_yz_kernel<1><<<h->sm_count * 8, 256, 0, h->stream>>>(st, xw, L);
+            else
+                ising::gather_lines_yz_kernel<2><<<h->sm_count * 8, 256, 0, h->stream>>>(st, xw, L);
+            ising::gram_kernel<<<h->sm_count, ising::kGramThreads, smem, h->stream>>>(
+                xw, h->d_gsum + ((size_t)rep * 3 + ax) * nr, h->d_queue + rep * 3 + ax, L, plan);
+            h->launches += 2;
+        }
+        ising::gram_finalize_kernel<<<(3 * nr + 255) / 256, 256, 0, h->stream>>>(
+            h->d_counts + (size_t)rep * cpr, h->d_gsum + (size_t)rep * 3 * nr, nr);
+        h->launches += 1;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return ISING3D_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -306,6 +362,17 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream)
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     h->stream = (cudaStream_t)cuda_stream;
+    return ISING3D_OK;
+}
+
+int ising3d_set_measure_variant(ising3d_t *h, int variant)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (variant < ISING3D_MEASURE_AUTO || variant > ISING3D_MEASURE_TENSOR)
+        return fail(ISING3D_EINVAL, "unknown measurement variant");
+    if (variant == ISING3D_MEASURE_TENSOR && !ising::gram_supported(h->L))
+        return fail(ISING3D_EINVAL, "the tensor-core measurement needs L to be a multiple of 512");
+    h->measure_variant = variant;
     return ISING3D_OK;
 }
 
@@ -384,6 +451,10 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
         ising::count_up_kernel<<<dim3(gx, h->n_rep), 256, 0, h->stream>>>(
             st, h->d_counts, h->words_per_replica(), cpr);
     }
+    if (h->use_gram()) {
+        const int rc = measure_gram(h);
+        if (rc != ISING3D_OK) return rc;
+    } else
     {
         // A_mu(r): persistent CTAs over tiles of C line-word sequences (kernels_measure.cuh)
         const int C = ising::autocorr_tile_sequences(L);
@@ -409,8 +480,9 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
                                                                                 n_tiles, cpr);
         ising::autocorr_kernel<2><<<grid, ising::kAcThreads, smem, h->stream>>>(st, h->d_counts, L, C,
                                                                                 n_tiles, cpr);
+        h->launches += 3;
     }
-    h->launches += 4;
+    h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     std::vector<unsigned long long> host((size_t)h->n_rep * cpr);
     CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_counts, host.size() * 8, cudaMemcpyDeviceToHost,
@@ -479,6 +551,12 @@ int ising3d_L(const ising3d_t *h) { return h ? h->L : 0; }
 int ising3d_n_rep(const ising3d_t *h) { return h ? h->n_rep : 0; }
 uint64_t ising3d_sweep_count(const ising3d_t *h) { return h ? h->sweep : 0; }
 uint64_t ising3d_launch_count(const ising3d_t *h) { return h ? h->launches : 0; }
+const char *ising3d_measure_variant_name(const ising3d_t *h)
+{
+    if (!h) return "none";
+    return h->use_gram() ? "tensor" : "popcount";
+}
+
 const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";

@@ -1,0 +1,358 @@
+// Tensor-core formulation of the pair counts a8 (D8) for large lattices (L a multiple of 512).
+//
+// Along one axis the lattice is a 0/1 matrix X[pos][line], pos = 0..L-1 the coordinate along
+// the axis, line = one of the L^2 lattice lines (1 <=> s = +1).  With the Gram matrix
+//     G[a][b] = sum_line X[a][line] * X[b][line]                     (a dense contraction, K = L^2)
+// the antiparallel-pair count of D8 is
+//     A(r) = sum_a sum_line [X[a] != X[a+r]] = 2 N_up - 2 sum_a G[a][(a + r) mod L],
+// exactly, in integers.  G is computed on the 5th-generation tensor cores: tcgen05.mma
+// kind::i8 (u8 x u8 -> s32 accumulators in tensor memory; |G| <= L^2 < 2^31), issued by one
+// thread, 128 x 128 x 32 per instruction.  The operands do not exist in memory as bytes: the
+// line bits are expanded to bytes by the CUDA cores straight into the 128-byte-swizzled K-major
+// shared-memory tiles the MMA reads (the expansion, 2 LOP3 + 1 PRMT-free IMAD per 4 bytes, is
+// what bounds the kernel together with the MMA itself).
+//
+// Three kernels:
+//   gather_lines_kernel<AX>  packed state (D3) -> Xw[pos][L^2/32] line words (bit = one line), in
+//                            the handle's spare ping-pong buffer: plane/row copies for z and y
+//                            (a site keeps its bit under a y/z shift and alternates colour), a
+//                            32x32 warp bit-transpose for x.
+//   gram_kernel              persistent CTAs, dynamic task queue; task = (128 positions a) x
+//                            (up to 4 units of 128 positions b = a0 + 128 u ...) x (a slice of K).
+//                            8 expander warps fill a 2-stage ring (full/empty mbarriers, generic
+//                            -> async proxy fence), warp 8 issues the MMAs and commits, the
+//                            expander warps read the accumulators back (tcgen05.ld) and add
+//                            G[a][b] to a shared-memory histogram over r = b - a.
+//   gram_finalize_kernel     A_mu(r) = 2 N_up - 2 Gsum_mu(r).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "kernels_fused.cuh"     // smem_u32, mbar_init, mbar_wait
+#include "kernels_measure.cuh"   // warp_transpose32
+
+namespace ising {
+
+constexpr int kGramExpWarps = 8;                       // expander / epilogue warps
+constexpr int kGramThreads = (kGramExpWarps + 1) * 32;   // + the MMA warp
+constexpr int kGramStages = 2;
+constexpr int kGramMaxUnits = 4;                       // 4 x 128 accumulator columns = all of TMEM
+constexpr int kGramTile = 128 * 128;                   // bytes of one 128-row operand tile (K = 128)
+
+inline bool gram_supported(int L) { return L >= 512 && (L % 512) == 0; }
+
+// ---- gather: packed state -> line words Xw[pos][RW], RW = L*L/32 ------------------------------
+// z: Xw[z][p*PW + i]          = W[(z+p)&1][z][i],            PW = L*L/64 plane words, i = y*WPR+wi
+// y: Xw[y][(p*L + z)*WPR + wi] = W[(y+p)&1][z][y][wi]
+template <int AX>
+__global__ void __launch_bounds__(256)
+gather_lines_yz_kernel(const uint32_t *__restrict__ state, uint32_t *__restrict__ xw, const int L)
+{
+    const int WPR = L >> 6;
+    const size_t PW = (size_t)L * WPR, WPC = PW * L, RW = 2 * PW;
+    const size_t n4 = (size_t)L * RW / 4;
+    for (size_t i4 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i4 < n4;
+         i4 += (size_t)gridDim.x * blockDim.x) {
+        const size_t o = i4 * 4;
+        const size_t pos = o / RW, lw = o - pos * RW;
+        size_t src;
+        if (AX == 2) {
+            const size_t p = lw / PW, i = lw - p * PW;
+            src = ((pos + p) & 1) * WPC + pos * PW + i;
+        } else {
+            const size_t p = lw / PW, rem = lw - p * PW;
+            const size_t z = rem / WPR, wi = rem - z * WPR;
+            src = ((pos + p) & 1) * WPC + (z * L + pos) * WPR + wi;
+        }
+        *reinterpret_cast<uint4 *>(xw + o) = *reinterpret_cast<const uint4 *>(state + src);
+    }
+}
+
+// x: Xw[x][z*(L/32) + yb] bit i = spin (x, 32 yb + i, z).  One block = (z, NWB consecutive words
+// of the rows = 64 NWB x-positions, all y); the transposed words go through shared memory so
+// that the stores are runs of L/32 consecutive line words.
+__global__ void __launch_bounds__(256)
+gather_lines_x_kernel(const uint32_t *__restrict__ state, uint32_t *__restrict__ xw, const int L,
+                      const int NWB)
+{
+    extern __shared__ uint32_t gx_smem[];              // [64 NWB x][L/32 + 1]
+    const int WPR = L >> 6, YB = L >> 5, LD = YB + 1;
+    const size_t PW = (size_t)L * WPR, WPC = PW * L, RW = 2 * PW;
+    const int z = blockIdx.x / (WPR / NWB), wi0 = (blockIdx.x % (WPR / NWB)) * NWB;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // job = (yb, w in 0..NWB-1, eo): lane = row 32 yb + lane
+    for (int job = warp; job < YB * 2 * NWB; job += 8) {
+        const int eo = job & 1, w = (job >> 1) % NWB, yb = job / (2 * NWB);
+        const int y = 32 * yb + lane;
+        const int col = (y + z + eo) & 1;
+        const uint32_t v = state[(size_t)col * WPC + ((size_t)z * L + y) * WPR + wi0 + w];
+        const uint32_t t = warp_transpose32(v, lane);  // lane j: bits over the 32 rows at k = 32(wi0+w)+j
+        gx_smem[(2 * (32 * w + lane) + eo) * LD + yb] = t;
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < 64 * NWB * YB; idx += 256) {
+        const int xl = idx / YB, yb = idx - xl * YB;
+        xw[(size_t)(64 * wi0 + xl) * RW + (size_t)z * YB + yb] = gx_smem[xl * LD + yb];
+    }
+}
+
+// ---- tcgen05 helpers ---------------------------------------------------------------------------
+// shared-memory matrix descriptor: K-major, SWIZZLE_128B (8 rows x 128 B atoms, 1024 B apart)
+__device__ __forceinline__ uint64_t umma_desc_k128(uint32_t saddr)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFF) >> 4);   // start address >> 4, bits [0,14)
+    d |= (uint64_t)1 << 16;                    // leading byte offset (unused for one K atom)
+    d |= (uint64_t)(1024 >> 4) << 32;          // stride byte offset: 8 rows x 128 B
+    d |= (uint64_t)1 << 46;                    // descriptor version (sm_100)
+    d |= (uint64_t)2 << 61;                    // SWIZZLE_128B
+    return d;
+}
+
+// instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, M = 128, N = 128
+constexpr uint32_t kGramIdesc = (2u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}\n"
+        ::"r"(tmem_d), "l"(da), "l"(db), "r"(kGramIdesc), "r"(accumulate)
+        : "memory");
+}
+
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+// 4 bits -> 4 bytes of 0/1 (bit i -> byte i): the four partial products land on distinct bits
+__device__ __forceinline__ uint32_t nibble_to_bytes(uint32_t n)
+{
+    return (n * 0x00204081u) & 0x01010101u;
+}
+
+// one row of a tile: 128 line bits (4 words) -> 128 bytes, 16-byte piece c stored at c ^ (row & 7)
+__device__ __forceinline__ void expand_row(uint8_t *tile, const int row, const uint4 w)
+{
+    const uint32_t in[4] = {w.x, w.y, w.z, w.w};
+    uint8_t *base = tile + row * 128;
+    const int sw = row & 7;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t ev = in[i] & 0x0F0F0F0Fu, od = (in[i] >> 4) & 0x0F0F0F0Fu;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {          // 16 bits -> 16 bytes
+            uint4 o;
+            o.x = nibble_to_bytes((ev >> (16 * h)) & 0xFFu);
+            o.y = nibble_to_bytes((od >> (16 * h)) & 0xFFu);
+            o.z = nibble_to_bytes((ev >> (16 * h + 8)) & 0xFFu);
+            o.w = nibble_to_bytes((od >> (16 * h + 8)) & 0xFFu);
+            *reinterpret_cast<uint4 *>(base + (((2 * i + h) ^ sw) << 4)) = o;
+        }
+    }
+}
+
+struct GramPlan {
+    int n_groups;            // column groups per row block
+    int units[8];            // units (of 128 columns) per group
+    int ustart[8];           // first unit of each group
+    int n_slices;            // K slices
+    int n_tasks;             // n_slices * (L/128) * n_groups
+};
+
+inline GramPlan make_gram_plan(int L, int sm_count)
+{
+    GramPlan p = {};
+    const int U = L / 256 + 1;                       // units covering b - a in [0, L/2 + 127]
+    p.n_groups = (U + kGramMaxUnits - 1) / kGramMaxUnits;
+    int u = 0;
+    for (int g = 0; g < p.n_groups; ++g) {
+        p.units[g] = U / p.n_groups + (g < U % p.n_groups ? 1 : 0);
+        p.ustart[g] = u;
+        u += p.units[g];
+    }
+    const int tiles = (L / 128) * p.n_groups;
+    p.n_slices = (sm_count * 12 + tiles - 1) / tiles;
+    p.n_tasks = p.n_slices * tiles;
+    return p;
+}
+
+inline size_t gram_smem_bytes(int L)
+{
+    return (size_t)kGramStages * (1 + kGramMaxUnits) * kGramTile + (size_t)(L / 2 + 1) * 4 + 1024 + 256;
+}
+
+// ---- the Gram kernel ---------------------------------------------------------------------------
+// xw: line words Xw[pos][RW]; gsum[r] += sum_a G[a][(a+r) mod L] for r = 1..L/2 (64-bit);
+// queue: task counter (zeroed by the host before the launch).
+__global__ void __launch_bounds__(kGramThreads, 1)
+gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gsum,
+            unsigned int *__restrict__ queue, const int L, const __grid_constant__ GramPlan plan)
+{
+    extern __shared__ __align__(1024) uint8_t gram_raw[];
+    uint8_t *smem = gram_raw + ((1024u - (smem_u32(gram_raw) & 1023u)) & 1023u);
+    // stage s: A tile, then kGramMaxUnits B tiles
+    uint8_t *tiles = smem;
+    uint32_t *hist = reinterpret_cast<uint32_t *>(smem + (size_t)kGramStages * (1 + kGramMaxUnits) * kGramTile);
+    __shared__ uint64_t full_bar[kGramStages], empty_bar[kGramStages], acc_full, acc_empty;
+    __shared__ uint32_t tmem_base_s;
+    __shared__ int task_s[2];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const size_t RW = (size_t)L * L / 32;
+    const int n_chunks = (int)(RW / 4);
+    const int half = L >> 1;
+    const int row_blocks = L / 128;
+    const int tiles_per_slice = row_blocks * plan.n_groups;
+
+    for (int r = tid; r <= half; r += kGramThreads) hist[r] = 0;
+    if (warp == kGramExpWarps) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         smem_u32(&tmem_base_s)), "r"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (tid == 0) {
+        for (int s = 0; s < kGramStages; ++s) {
+            mbar_init(smem_u32(&full_bar[s]), kGramExpWarps);
+            mbar_init(smem_u32(&empty_bar[s]), 1);
+        }
+        mbar_init(smem_u32(&acc_full), 1);
+        mbar_init(smem_u32(&acc_empty), kGramExpWarps);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        task_s[0] = (int)atomicAdd(queue, 1u);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem_base = tmem_base_s;
+
+    uint32_t it = 0;                                   // chunk counter over all tasks (ring position)
+    int n_done = 0;                                    // tasks finished by this CTA
+    for (int task = task_s[0]; task < plan.n_tasks; ++n_done) {
+        // decode: slice-major so that concurrently running CTAs read the same K range (L2 reuse)
+        const int slice = task / tiles_per_slice, tl = task - slice * tiles_per_slice;
+        const int rb = tl / plan.n_groups, grp = tl - rb * plan.n_groups;
+        const int a0 = rb * 128, nu = plan.units[grp], us = plan.ustart[grp];
+        const int b0 = a0 + 128 * us;
+        const int c_begin = (int)((long long)n_chunks * slice / plan.n_slices);
+        const int c_end = (int)((long long)n_chunks * (slice + 1) / plan.n_slices);
+        const bool share_a = us == 0;                  // unit 0 of the group is the A tile itself
+        const int n_rows = 128 + 128 * (share_a ? nu - 1 : nu);
+
+        if (warp < kGramExpWarps) {
+            // ------------------------------------------------ expanders
+            for (int c = c_begin; c < c_end; ++c, ++it) {
+                const int s = it & (kGramStages - 1);
+                mbar_wait(smem_u32(&empty_bar[s]), ((it / kGramStages) & 1) ^ 1);
+                uint8_t *stage = tiles + (size_t)s * (1 + kGramMaxUnits) * kGramTile;
+                for (int row = tid; row < n_rows; row += kGramExpWarps * 32) {
+                    // rows 0..127: A (positions a0 + row); then the B units not shared with A
+                    int pos, trow;
+                    uint8_t *tile;
+                    if (row < 128) {
+                        pos = a0 + row;
+                        tile = stage;
+                        trow = row;
+                    } else {
+                        const int ub = (row >> 7) - 1 + (share_a ? 1 : 0);     // unit inside the group
+                        trow = row & 127;
+                        pos = b0 + 128 * ub + trow;
+                        tile = stage + (size_t)(1 + ub) * kGramTile;
+                    }
+                    if (pos >= L) pos -= L;
+                    const uint4 w = *reinterpret_cast<const uint4 *>(xw + (size_t)pos * RW + 4 * (size_t)c);
+                    expand_row(tile, trow, w);
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&full_bar[s]));
+            }
+            // ------------------------------------------------ epilogue: G[a][b] -> hist[b - a]
+            mbar_wait(smem_u32(&acc_full), (uint32_t)(n_done & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            {
+                const int lrow = 32 * (warp & 3) + lane;           // TMEM lane = row of the tile
+                const int ncol = 128 * nu, chalf = ncol / 2;
+                const int cbeg = (warp >> 2) * chalf;
+                for (int c0 = cbeg; c0 < cbeg + chalf; c0 += 16) {
+                    uint32_t v[16];
+                    const uint32_t taddr = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)c0;
+                    asm volatile(
+                        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+                          "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]),
+                          "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                        : "r"(taddr));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const int r = 128 * us + c0 + j - lrow;    // b - a (before the periodic wrap)
+                        if (r >= 1 && r <= half) atomicAdd(&hist[r], v[j]);
+                    }
+                }
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&acc_empty));
+        } else {
+            // ------------------------------------------------ MMA issuer (one thread)
+            if (lane == 0) {
+                if (n_done > 0) {
+                    mbar_wait(smem_u32(&acc_empty), (uint32_t)((n_done - 1) & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;");
+                }
+                uint32_t itm = it;
+                for (int c = c_begin; c < c_end; ++c, ++itm) {
+                    const int s = itm & (kGramStages - 1);
+                    mbar_wait(smem_u32(&full_bar[s]), (itm / kGramStages) & 1);
+                    asm volatile("tcgen05.fence::after_thread_sync;");
+                    const uint32_t sbase = smem_u32(tiles + (size_t)s * (1 + kGramMaxUnits) * kGramTile);
+                    const uint64_t da = umma_desc_k128(sbase);
+                    for (int u = 0; u < nu; ++u) {
+                        const uint64_t db = (share_a && u == 0) ? da
+                                                                : umma_desc_k128(sbase + (uint32_t)(1 + u) * kGramTile);
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks)         // K = 32 per instruction: +32 B in the atom
+                            umma_i8(tmem_base + (uint32_t)(128 * u), da + (uint64_t)(2 * ks),
+                                    db + (uint64_t)(2 * ks), (c > c_begin || ks > 0) ? 1u : 0u);
+                    }
+                    umma_commit(smem_u32(&empty_bar[s]));      // frees the stage when the MMAs have read it
+                }
+                umma_commit(smem_u32(&acc_full));              // accumulators of this task complete
+            }
+            it += (uint32_t)(c_end - c_begin);
+            __syncwarp();
+        }
+        // next task (one fetch per CTA, broadcast through shared memory)
+        if (tid == 0) task_s[(n_done + 1) & 1] = (int)atomicAdd(queue, 1u);
+        __syncthreads();
+        task = task_s[(n_done + 1) & 1];
+    }
+
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    for (int r = 1 + tid; r <= half; r += kGramThreads)
+        if (hist[r]) atomicAdd(&gsum[r], (unsigned long long)hist[r]);
+    if (warp == kGramExpWarps)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512));
+}
+
+// A_mu(r) = 2 N_up - 2 Gsum_mu(r) for r = 1..L/2 (counts layout of kernels_measure.cuh)
+__global__ void gram_finalize_kernel(unsigned long long *__restrict__ counts,
+                                     const unsigned long long *__restrict__ gsum, const int nr)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 3 * nr) return;
+    const int r = i % nr;
+    counts[1 + i] = r == 0 ? 0ull : 2ull * counts[0] - 2ull * gsum[i];
+}
+
+}  // namespace ising

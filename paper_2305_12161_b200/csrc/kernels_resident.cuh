@@ -22,6 +22,7 @@
 // keys live in registers.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
@@ -126,32 +127,41 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
     uint4 *peer_up = cluster.map_shared_rank(res_smem, rank_up);   // its slot 0    <- my plane PZ-1
     cluster.sync();                               // everybody loaded; peers' smem exists
 
+    // one half-sweep of compile-time colour C (the compiler then folds the colour into the
+    // smem offsets and the Philox counter)
+    auto half_sweep = [&](auto colour, const uint32_t t) {
+        constexpr int C = decltype(colour)::value;
+        uint4 *own = res_smem + (size_t)C * CSTRIDE;
+        const uint4 *oth = res_smem + (size_t)(1 - C) * CSTRIDE;
+        if (active) {
+            for (int zl = pl; zl < PZ; zl += PPI) {
+                const int z = z0 + zl;
+                const uint4 *pz = oth + (size_t)(zl + 1) * GPP;
+                const uint4 sam = pz[g], prv = pz[g_prev], nxt = pz[g_next];
+                const uint4 zm = pz[g - GPP], zp = pz[g + GPP];
+                const uint4 o4 = own[(size_t)(zl + 1) * GPP + g];
+                const uint32_t q = (uint32_t)z * GPP + g;
+                const uint4 rho = philox4x32_10(q, t, (uint32_t)C, kTagTie, keys);
+                const uint4 nw = res_update_group<WPR>(o4, prv, sam, nxt, zm, zp, rho, (y0 + z + C) & 1);
+                own[(size_t)(zl + 1) * GPP + g] = nw;
+                if (zl == 0) peer_dn[(size_t)C * CSTRIDE + (size_t)(PZ + 1) * GPP + g] = nw;
+                if (zl == PZ - 1) peer_up[(size_t)C * CSTRIDE + g] = nw;
+            }
+        }
+        cluster.sync();
+    };
+    using Colour0 = std::integral_constant<int, 0>;
+    using Colour1 = std::integral_constant<int, 1>;
+
     for (uint32_t it = 0; it < n_sweeps; ++it) {
         const uint32_t t = t0 + it;
         // 01 cycle: colour 0 first (D7); mixed cycle: the first colour is drawn per sweep (D10)
-        const int first = mixed ? first_colour(seed, t) : 0;
-#pragma unroll 1
-        for (int phase = 0; phase < 2; ++phase) {
-            const int c = phase ^ first;
-            uint4 *own = res_smem + (size_t)c * CSTRIDE;
-            const uint4 *oth = res_smem + (size_t)(1 - c) * CSTRIDE;
-            if (active) {
-                for (int zl = pl; zl < PZ; zl += PPI) {
-                    const int z = z0 + zl;
-                    const uint4 *pz = oth + (size_t)(zl + 1) * GPP;
-                    const uint4 sam = pz[g], prv = pz[g_prev], nxt = pz[g_next];
-                    const uint4 zm = pz[g - GPP], zp = pz[g + GPP];
-                    const uint4 o4 = own[(size_t)(zl + 1) * GPP + g];
-                    const uint32_t q = (uint32_t)z * GPP + g;
-                    const uint4 rho = philox4x32_10(q, t, (uint32_t)c, kTagTie, keys);
-                    const uint4 nw = res_update_group<WPR>(o4, prv, sam, nxt, zm, zp, rho,
-                                                           (y0 + z + c) & 1);
-                    own[(size_t)(zl + 1) * GPP + g] = nw;
-                    if (zl == 0) peer_dn[(size_t)c * CSTRIDE + (size_t)(PZ + 1) * GPP + g] = nw;
-                    if (zl == PZ - 1) peer_up[(size_t)c * CSTRIDE + g] = nw;
-                }
-            }
-            cluster.sync();
+        if (mixed && first_colour(seed, t)) {
+            half_sweep(Colour1{}, t);
+            half_sweep(Colour0{}, t);
+        } else {
+            half_sweep(Colour0{}, t);
+            half_sweep(Colour1{}, t);
         }
     }
 

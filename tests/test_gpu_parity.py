@@ -367,3 +367,54 @@ def test_library_owned_memory_and_errors(B, orc):
     sim.free()
     with pytest.raises(B.Ising3DError):
         B.Ising3D(100, [1])
+
+
+# ------------------------------------------------------------------ measurement kernels: tensor vs popcount
+def test_tensor_measurement_against_oracle(B, orc):
+    """tcgen05 Gram-matrix pair counts (L % 512 == 0) against the oracle's triple loops."""
+    L, seed = 512, 11
+    sim = B.Ising3D(L, [seed])
+    assert sim.measure_variant_name == "tensor"
+    ref = orc.Oracle(L, seed)
+    check_measure(sim.measure(), ref.measure_full())          # T = infinity start
+    sim.sweep(3)
+    ref.sweep(3)
+    check_measure(sim.measure(), ref.measure_full())
+    sim.set_measure_variant(B.MEASURE_POPCOUNT)
+    assert sim.measure_variant_name == "popcount"
+    check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+
+
+@pytest.mark.parametrize("L", [512, 1024, 2048])
+def test_tensor_equals_popcount_measurement(B, L):
+    """Both measurement paths give the same integers at sizes the oracle cannot reach in full;
+    the popcount path is oracle-checked at L <= 512 and on thinned r sets at L = 1024."""
+    sim = B.Ising3D(L, [5])
+    for n in (0, 2):
+        sim.sweep(n)
+        sim.set_measure_variant(B.MEASURE_TENSOR)
+        a = sim.measure()
+        sim.set_measure_variant(B.MEASURE_POPCOUNT)
+        b = sim.measure()
+        assert np.array_equal(a["antipar"], b["antipar"]) and np.array_equal(a["n_up"], b["n_up"])
+        assert np.array_equal(a["C"], b["C"])
+    # structured input: coarse domains
+    if L <= 1024:
+        sim.set_state(inputs.coarse_words(L, 3, block=16), 7)
+        sim.set_measure_variant(B.MEASURE_TENSOR)
+        a = sim.measure()
+        sim.set_measure_variant(B.MEASURE_POPCOUNT)
+        b = sim.measure()
+        assert np.array_equal(a["antipar"], b["antipar"])
+    sim.free()
+
+
+def test_measure_variant_errors(B):
+    sim = B.Ising3D(256, [1])
+    assert sim.measure_variant_name == "popcount"
+    with pytest.raises(B.Ising3DError):
+        sim.set_measure_variant(B.MEASURE_TENSOR)
+    with pytest.raises(B.Ising3DError):
+        sim.set_measure_variant(9)
+    sim.free()
