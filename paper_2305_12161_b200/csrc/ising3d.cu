@@ -281,17 +281,18 @@ int measure_gram(ising3d *h)
 {
     const int L = h->L, nr = L / 2 + 1, cpr = h->counts_per_replica();
     static bool attr_set = false;
-    const size_t smem = ising::gram_smem_bytes(L);
-    const int NWB = L <= 2048 ? 8 : 4;
-    const size_t smem_x = (size_t)64 * NWB * (L / 32 + 1) * 4;
+    const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
+    const size_t smem = ising::gram_smem_bytes(L, plan);
+    int NWB = 4;
+    if (const char *e = getenv("ISING3D_GATHER_NWB")) NWB = atoi(e);   // experiments only
+    const size_t smem_x = ((size_t)64 * NWB * (L / 32 + 1) + (size_t)2 * 256 * (NWB + 1)) * 4;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(ising::gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)ising::gram_smem_bytes(4096)));
+                                      210 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(ising::gather_lines_x_kernel,
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024));
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
         attr_set = true;
     }
-    const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
     CUDA_TRY(cudaMemsetAsync(h->d_gsum, 0, (size_t)h->n_rep * 3 * nr * 8, h->stream));
     CUDA_TRY(cudaMemsetAsync(h->d_queue, 0, (size_t)h->n_rep * 3 * 4, h->stream));
     const size_t wpr = h->words_per_replica();

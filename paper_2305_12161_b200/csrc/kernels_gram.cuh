@@ -34,8 +34,9 @@
 namespace ising {
 
 constexpr int kGramExpWarps = 8;                       // expander / epilogue warps
+constexpr int kGramRowsPerThread = (128 * (1 + 4) + kGramExpWarps * 32 - 1) / (kGramExpWarps * 32);
 constexpr int kGramThreads = (kGramExpWarps + 1) * 32;   // + the MMA warp
-constexpr int kGramStages = 2;
+constexpr int kGramMaxStages = 3;
 constexpr int kGramMaxUnits = 4;                       // 4 x 128 accumulator columns = all of TMEM
 constexpr int kGramTile = 128 * 128;                   // bytes of one 128-row operand tile (K = 128)
 
@@ -75,21 +76,30 @@ __global__ void __launch_bounds__(256)
 gather_lines_x_kernel(const uint32_t *__restrict__ state, uint32_t *__restrict__ xw, const int L,
                       const int NWB)
 {
-    extern __shared__ uint32_t gx_smem[];              // [64 NWB x][L/32 + 1]
-    const int WPR = L >> 6, YB = L >> 5, LD = YB + 1;
+    extern __shared__ uint32_t gx_smem[];              // out [64 NWB x][L/32 + 1], raw [2][256][NWB + 1]
+    const int WPR = L >> 6, YB = L >> 5, LD = YB + 1, RD = NWB + 1;
     const size_t PW = (size_t)L * WPR, WPC = PW * L, RW = 2 * PW;
     const int z = blockIdx.x / (WPR / NWB), wi0 = (blockIdx.x % (WPR / NWB)) * NWB;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // job = (yb, w in 0..NWB-1, eo): lane = row 32 yb + lane
-    for (int job = warp; job < YB * 2 * NWB; job += 8) {
-        const int eo = job & 1, w = (job >> 1) % NWB, yb = job / (2 * NWB);
-        const int y = 32 * yb + lane;
-        const int col = (y + z + eo) & 1;
-        const uint32_t v = state[(size_t)col * WPC + ((size_t)z * L + y) * WPR + wi0 + w];
-        const uint32_t t = warp_transpose32(v, lane);  // lane j: bits over the 32 rows at k = 32(wi0+w)+j
-        gx_smem[(2 * (32 * w + lane) + eo) * LD + yb] = t;
+    uint32_t *raw = gx_smem + (size_t)64 * NWB * LD;
+    for (int y0 = 0; y0 < L; y0 += 256) {
+        // both colours of rows y0..y0+255, words wi0..wi0+NWB-1: runs of NWB words (coalesced)
+        for (int idx = threadIdx.x; idx < 2 * 256 * NWB; idx += 256) {
+            const int w = idx % NWB, yl = (idx / NWB) & 255, col = idx / (NWB * 256);
+            raw[(col * 256 + yl) * RD + w] =
+                state[(size_t)col * WPC + ((size_t)z * L + y0 + yl) * WPR + wi0 + w];
+        }
+        __syncthreads();
+        // job = (yb in the batch, w, eo): lane = row 32 yb + lane; even-x sites sit in colour (y+z)&1
+        for (int job = warp; job < 8 * 2 * NWB; job += 8) {
+            const int eo = job & 1, w = (job >> 1) % NWB, ybl = job / (2 * NWB);
+            const int yl = 32 * ybl + lane;
+            const int col = (y0 + yl + z + eo) & 1;
+            const uint32_t t = warp_transpose32(raw[(col * 256 + yl) * RD + w], lane);
+            gx_smem[(2 * (32 * w + lane) + eo) * LD + (y0 >> 5) + ybl] = t;   // lane j: k = 32 w + j
+        }
+        __syncthreads();
     }
-    __syncthreads();
     for (int idx = threadIdx.x; idx < 64 * NWB * YB; idx += 256) {
         const int xl = idx / YB, yb = idx - xl * YB;
         xw[(size_t)(64 * wi0 + xl) * RW + (size_t)z * YB + yb] = gx_smem[xl * LD + yb];
@@ -111,13 +121,15 @@ __device__ __forceinline__ uint64_t umma_desc_k128(uint32_t saddr)
 
 // instruction descriptor, kind::i8: D = s32, A = B = u8, both K-major, M = 128, N = 128
 constexpr uint32_t kGramIdesc = (2u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+constexpr uint32_t kGramIdesc256 = (2u << 4) | ((256u >> 3) << 17) | ((128u >> 4) << 24);   // N = 256
 
-__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t accumulate)
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc,
+                                        uint32_t accumulate)
 {
     asm volatile(
         "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}\n"
-        ::"r"(tmem_d), "l"(da), "l"(db), "r"(kGramIdesc), "r"(accumulate)
+        ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 
@@ -163,6 +175,8 @@ struct GramPlan {
     int n_groups;            // column groups per row block
     int units[8];            // units (of 128 columns) per group
     int ustart[8];           // first unit of each group
+    int max_units;           // largest group: a stage is (1 + max_units) tiles
+    int n_stages;            // ring depth (2 or 3, what fits shared memory)
     int n_slices;            // K slices
     int n_tasks;             // n_slices * (L/128) * n_groups
 };
@@ -178,15 +192,17 @@ inline GramPlan make_gram_plan(int L, int sm_count)
         p.ustart[g] = u;
         u += p.units[g];
     }
+    p.max_units = p.units[0];
+    p.n_stages = (1 + p.max_units) * kGramTile * 3 <= 196 * 1024 ? 3 : 2;
     const int tiles = (L / 128) * p.n_groups;
     p.n_slices = (sm_count * 12 + tiles - 1) / tiles;
     p.n_tasks = p.n_slices * tiles;
     return p;
 }
 
-inline size_t gram_smem_bytes(int L)
+inline size_t gram_smem_bytes(int L, const GramPlan &p)
 {
-    return (size_t)kGramStages * (1 + kGramMaxUnits) * kGramTile + (size_t)(L / 2 + 1) * 4 + 1024 + 256;
+    return (size_t)p.n_stages * (1 + p.max_units) * kGramTile + (size_t)(L / 2 + 1) * 4 + 1024 + 256;
 }
 
 // ---- the Gram kernel ---------------------------------------------------------------------------
@@ -198,10 +214,12 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
 {
     extern __shared__ __align__(1024) uint8_t gram_raw[];
     uint8_t *smem = gram_raw + ((1024u - (smem_u32(gram_raw) & 1023u)) & 1023u);
-    // stage s: A tile, then kGramMaxUnits B tiles
+    // stage s: A tile, then max_units B tiles
     uint8_t *tiles = smem;
-    uint32_t *hist = reinterpret_cast<uint32_t *>(smem + (size_t)kGramStages * (1 + kGramMaxUnits) * kGramTile);
-    __shared__ uint64_t full_bar[kGramStages], empty_bar[kGramStages], acc_full, acc_empty;
+    const int NS = plan.n_stages;
+    const size_t stage_bytes = (size_t)(1 + plan.max_units) * kGramTile;
+    uint32_t *hist = reinterpret_cast<uint32_t *>(smem + (size_t)NS * stage_bytes);
+    __shared__ uint64_t full_bar[kGramMaxStages], empty_bar[kGramMaxStages], acc_full, acc_empty;
     __shared__ uint32_t tmem_base_s;
     __shared__ int task_s[2];
 
@@ -219,7 +237,7 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     if (tid == 0) {
-        for (int s = 0; s < kGramStages; ++s) {
+        for (int s = 0; s < NS; ++s) {
             mbar_init(smem_u32(&full_bar[s]), kGramExpWarps);
             mbar_init(smem_u32(&empty_bar[s]), 1);
         }
@@ -233,7 +251,9 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem_base = tmem_base_s;
 
-    uint32_t it = 0;                                   // chunk counter over all tasks (ring position)
+    uint32_t it = 0;                                   // chunk counter over all tasks
+    int rs = 0;                                        // ring position: stage rs, wrap parity rp
+    uint32_t rp = 0;
     int n_done = 0;                                    // tasks finished by this CTA
     for (int task = task_s[0]; task < plan.n_tasks; ++n_done) {
         // decode: slice-major so that concurrently running CTAs read the same K range (L2 reuse)
@@ -248,38 +268,61 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
 
         if (warp < kGramExpWarps) {
             // ------------------------------------------------ expanders
-            for (int c = c_begin; c < c_end; ++c, ++it) {
-                const int s = it & (kGramStages - 1);
-                mbar_wait(smem_u32(&empty_bar[s]), ((it / kGramStages) & 1) ^ 1);
-                uint8_t *stage = tiles + (size_t)s * (1 + kGramMaxUnits) * kGramTile;
-                for (int row = tid; row < n_rows; row += kGramExpWarps * 32) {
-                    // rows 0..127: A (positions a0 + row); then the B units not shared with A
-                    int pos, trow;
-                    uint8_t *tile;
-                    if (row < 128) {
-                        pos = a0 + row;
-                        tile = stage;
-                        trow = row;
-                    } else {
-                        const int ub = (row >> 7) - 1 + (share_a ? 1 : 0);     // unit inside the group
-                        trow = row & 127;
-                        pos = b0 + 128 * ub + trow;
-                        tile = stage + (size_t)(1 + ub) * kGramTile;
-                    }
-                    if (pos >= L) pos -= L;
-                    const uint4 w = *reinterpret_cast<const uint4 *>(xw + (size_t)pos * RW + 4 * (size_t)c);
-                    expand_row(tile, trow, w);
+            // this thread's rows (at most kGramRowsPerThread of up to 640): tile, row inside the tile, source row
+            constexpr int RPT = kGramRowsPerThread;
+            uint8_t *t_tile[RPT];
+            int t_row[RPT];
+            const uint32_t *t_src[RPT];
+            bool t_ok[RPT];
+#pragma unroll
+            for (int i = 0; i < RPT; ++i) {
+                const int row = tid + i * kGramExpWarps * 32;
+                t_ok[i] = row < n_rows;
+                // rows 0..127: A (positions a0 + row); then the B units not shared with A
+                int pos, ub = -1;
+                if (row < 128) {
+                    pos = a0 + row;
+                } else {
+                    ub = (row >> 7) - 1 + (share_a ? 1 : 0);               // unit inside the group
+                    pos = b0 + 128 * ub + (row & 127);
                 }
+                if (pos >= L) pos -= L;
+                if (pos >= L) pos -= L;                                    // rows past n_rows: harmless
+                // tile slots of a stage: slot 0 = A; unit u of B = slot u if it shares A (u = 0 is A
+                // itself), else slot 1 + u: the units of a group are contiguous either way
+                t_tile[i] = tiles + (size_t)(ub < 0 ? 0 : (share_a ? ub : 1 + ub)) * kGramTile;   // + stage offset later
+                t_row[i] = row & 127;
+                t_src[i] = xw + (size_t)pos * RW;
+            }
+            uint4 wn[RPT];                                                   // prefetched line words
+#pragma unroll
+            for (int i = 0; i < RPT; ++i)
+                if (t_ok[i]) wn[i] = *reinterpret_cast<const uint4 *>(t_src[i] + 4 * (size_t)c_begin);
+            for (int c = c_begin; c < c_end; ++c, ++it) {
+                uint4 wc[RPT];
+#pragma unroll
+                for (int i = 0; i < RPT; ++i) wc[i] = wn[i];
+                if (c + 1 < c_end) {
+#pragma unroll
+                    for (int i = 0; i < RPT; ++i)
+                        if (t_ok[i]) wn[i] = *reinterpret_cast<const uint4 *>(t_src[i] + 4 * (size_t)(c + 1));
+                }
+                mbar_wait(smem_u32(&empty_bar[rs]), rp ^ 1);
+                const size_t soff = (size_t)rs * stage_bytes;
+#pragma unroll
+                for (int i = 0; i < RPT; ++i)
+                    if (t_ok[i]) expand_row(t_tile[i] + soff, t_row[i], wc[i]);
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&full_bar[s]));
+                if (lane == 0) mbar_arrive(smem_u32(&full_bar[rs]));
+                if (++rs == NS) { rs = 0; rp ^= 1; }
             }
             // ------------------------------------------------ epilogue: G[a][b] -> hist[b - a]
             mbar_wait(smem_u32(&acc_full), (uint32_t)(n_done & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
             {
                 const int lrow = 32 * (warp & 3) + lane;           // TMEM lane = row of the tile
-                const int ncol = 128 * nu, chalf = ncol / 2;
+                const int ncol = 128 * nu, chalf = ncol / (kGramExpWarps / 4);
                 const int cbeg = (warp >> 2) * chalf;
                 for (int c0 = cbeg; c0 < cbeg + chalf; c0 += 16) {
                     uint32_t v[16];
@@ -309,26 +352,36 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
                     mbar_wait(smem_u32(&acc_empty), (uint32_t)((n_done - 1) & 1));
                     asm volatile("tcgen05.fence::after_thread_sync;");
                 }
-                uint32_t itm = it;
-                for (int c = c_begin; c < c_end; ++c, ++itm) {
-                    const int s = itm & (kGramStages - 1);
-                    mbar_wait(smem_u32(&full_bar[s]), (itm / kGramStages) & 1);
+                int ms = rs;
+                uint32_t mp = rp;
+                for (int c = c_begin; c < c_end; ++c) {
+                    const int s = ms;
+                    mbar_wait(smem_u32(&full_bar[s]), mp);
+                    if (++ms == NS) { ms = 0; mp ^= 1; }
                     asm volatile("tcgen05.fence::after_thread_sync;");
-                    const uint32_t sbase = smem_u32(tiles + (size_t)s * (1 + kGramMaxUnits) * kGramTile);
+                    const uint32_t sbase = smem_u32(tiles + (size_t)s * stage_bytes);
                     const uint64_t da = umma_desc_k128(sbase);
-                    for (int u = 0; u < nu; ++u) {
-                        const uint64_t db = (share_a && u == 0) ? da
-                                                                : umma_desc_k128(sbase + (uint32_t)(1 + u) * kGramTile);
+                    const uint32_t bslot0 = share_a ? 0u : 1u;
+                    for (int u = 0; u < nu; u += 2) {          // two units (N = 256) per instruction where possible
+                        const uint64_t db = umma_desc_k128(sbase + (bslot0 + (uint32_t)u) * kGramTile);
+                        const uint32_t idesc = (u + 1 < nu) ? kGramIdesc256 : kGramIdesc;
 #pragma unroll
                         for (int ks = 0; ks < 4; ++ks)         // K = 32 per instruction: +32 B in the atom
                             umma_i8(tmem_base + (uint32_t)(128 * u), da + (uint64_t)(2 * ks),
-                                    db + (uint64_t)(2 * ks), (c > c_begin || ks > 0) ? 1u : 0u);
+                                    db + (uint64_t)(2 * ks), idesc, (c > c_begin || ks > 0) ? 1u : 0u);
                     }
                     umma_commit(smem_u32(&empty_bar[s]));      // frees the stage when the MMAs have read it
                 }
                 umma_commit(smem_u32(&acc_full));              // accumulators of this task complete
             }
-            it += (uint32_t)(c_end - c_begin);
+            // all lanes of the MMA warp advance the ring position like the expanders did
+            {
+                const int adv = c_end - c_begin;
+                it += (uint32_t)adv;
+                const int tot = rs + adv;
+                if ((tot / NS) & 1) rp ^= 1;
+                rs = tot % NS;
+            }
             __syncwarp();
         }
         // next task (one fetch per CTA, broadcast through shared memory)
