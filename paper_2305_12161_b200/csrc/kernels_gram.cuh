@@ -9,8 +9,7 @@
 // kind::i8 (u8 x u8 -> s32 accumulators in tensor memory; |G| <= L^2 < 2^31), issued by one
 // thread, 128 x 128 x 32 per instruction.  The operands do not exist in memory as bytes: the
 // line bits are expanded to bytes by the CUDA cores straight into the 128-byte-swizzled K-major
-// shared-memory tiles the MMA reads (the expansion, 2 LOP3 + 1 PRMT-free IMAD per 4 bytes, is
-// what bounds the kernel together with the MMA itself).
+// shared-memory tiles the MMA reads (one LOP3 per 4 bytes, see expand_row).
 //
 // Three kernels:
 //   gather_lines_kernel<AX>  packed state (D3) -> Xw[pos][L^2/32] line words (bit = one line), in
@@ -144,13 +143,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
-// 4 bits -> 4 bytes of 0/1 (bit i -> byte i): the four partial products land on distinct bits
-__device__ __forceinline__ uint32_t nibble_to_bytes(uint32_t n)
-{
-    return (n * 0x00204081u) & 0x01010101u;
-}
-
-// one row of a tile: 128 line bits (4 words) -> 128 bytes, 16-byte piece c stored at c ^ (row & 7)
+// One row of a tile: 128 line bits (4 words) -> 128 bytes, 16-byte piece c stored at c ^ (row & 7).
+// The contraction index may be permuted freely as long as A and B agree, and the byte VALUES may
+// differ between A and B as long as every product of two set bytes is the same constant.  So:
+//   A row: byte-swapped word & (0x01010101 << j)        -> bytes in {0, 2^j}
+//   B row: bit-reversed word  & (0x01010101 << (7 - j)) -> bytes in {0, 2^(7-j)}, same line per byte
+// for j = 0..7: one PRMT or BREV plus eight LOP3 per 32 lines, no shifts, no multiplies, and every
+// product is 2^7: the accumulators hold 128 * G exactly (per task 128 * 128 * K_slice < 2^31).
+template <bool IS_B>
 __device__ __forceinline__ void expand_row(uint8_t *tile, const int row, const uint4 w)
 {
     const uint32_t in[4] = {w.x, w.y, w.z, w.w};
@@ -158,18 +158,19 @@ __device__ __forceinline__ void expand_row(uint8_t *tile, const int row, const u
     const int sw = row & 7;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const uint32_t ev = in[i] & 0x0F0F0F0Fu, od = (in[i] >> 4) & 0x0F0F0F0Fu;
+        const uint32_t v = IS_B ? __brev(in[i]) : __byte_perm(in[i], 0u, 0x0123u);
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {          // 16 bits -> 16 bytes
+        for (int h = 0; h < 2; ++h) {
             uint4 o;
-            o.x = nibble_to_bytes((ev >> (16 * h)) & 0xFFu);
-            o.y = nibble_to_bytes((od >> (16 * h)) & 0xFFu);
-            o.z = nibble_to_bytes((ev >> (16 * h + 8)) & 0xFFu);
-            o.w = nibble_to_bytes((od >> (16 * h + 8)) & 0xFFu);
+            o.x = v & (0x01010101u << (IS_B ? 7 - (4 * h + 0) : 4 * h + 0));
+            o.y = v & (0x01010101u << (IS_B ? 7 - (4 * h + 1) : 4 * h + 1));
+            o.z = v & (0x01010101u << (IS_B ? 7 - (4 * h + 2) : 4 * h + 2));
+            o.w = v & (0x01010101u << (IS_B ? 7 - (4 * h + 3) : 4 * h + 3));
             *reinterpret_cast<uint4 *>(base + (((2 * i + h) ^ sw) << 4)) = o;
         }
     }
 }
+constexpr int kGramProductShift = 7;       // accumulators = G << 7
 
 struct GramPlan {
     int n_groups;            // column groups per row block
@@ -263,8 +264,7 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
         const int b0 = a0 + 128 * us;
         const int c_begin = (int)((long long)n_chunks * slice / plan.n_slices);
         const int c_end = (int)((long long)n_chunks * (slice + 1) / plan.n_slices);
-        const bool share_a = us == 0;                  // unit 0 of the group is the A tile itself
-        const int n_rows = 128 + 128 * (share_a ? nu - 1 : nu);
+        const int n_rows = 128 + 128 * nu;             // A rows, then the B rows of the nu units
 
         if (warp < kGramExpWarps) {
             // ------------------------------------------------ expanders
@@ -278,19 +278,17 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
             for (int i = 0; i < RPT; ++i) {
                 const int row = tid + i * kGramExpWarps * 32;
                 t_ok[i] = row < n_rows;
-                // rows 0..127: A (positions a0 + row); then the B units not shared with A
+                // rows 0..127: A (positions a0 + row); then the B units (positions b0 + ...)
                 int pos, ub = -1;
                 if (row < 128) {
                     pos = a0 + row;
                 } else {
-                    ub = (row >> 7) - 1 + (share_a ? 1 : 0);               // unit inside the group
+                    ub = (row >> 7) - 1;                                   // unit inside the group
                     pos = b0 + 128 * ub + (row & 127);
                 }
                 if (pos >= L) pos -= L;
                 if (pos >= L) pos -= L;                                    // rows past n_rows: harmless
-                // tile slots of a stage: slot 0 = A; unit u of B = slot u if it shares A (u = 0 is A
-                // itself), else slot 1 + u: the units of a group are contiguous either way
-                t_tile[i] = tiles + (size_t)(ub < 0 ? 0 : (share_a ? ub : 1 + ub)) * kGramTile;   // + stage offset later
+                t_tile[i] = tiles + (size_t)(1 + ub) * kGramTile;   // slot 0 = A, slot 1 + u = unit u
                 t_row[i] = row & 127;
                 t_src[i] = xw + (size_t)pos * RW;
             }
@@ -311,7 +309,12 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
                 const size_t soff = (size_t)rs * stage_bytes;
 #pragma unroll
                 for (int i = 0; i < RPT; ++i)
-                    if (t_ok[i]) expand_row(t_tile[i] + soff, t_row[i], wc[i]);
+                    if (t_ok[i]) {
+                        if (tid + i * kGramExpWarps * 32 < 128)
+                            expand_row<false>(t_tile[i] + soff, t_row[i], wc[i]);
+                        else
+                            expand_row<true>(t_tile[i] + soff, t_row[i], wc[i]);
+                    }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&full_bar[rs]));
@@ -338,7 +341,7 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         const int r = 128 * us + c0 + j - lrow;    // b - a (before the periodic wrap)
-                        if (r >= 1 && r <= half) atomicAdd(&hist[r], v[j]);
+                        if (r >= 1 && r <= half) atomicAdd(&hist[r], v[j] >> kGramProductShift);
                     }
                 }
             }
@@ -361,9 +364,8 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const uint32_t sbase = smem_u32(tiles + (size_t)s * stage_bytes);
                     const uint64_t da = umma_desc_k128(sbase);
-                    const uint32_t bslot0 = share_a ? 0u : 1u;
                     for (int u = 0; u < nu; u += 2) {          // two units (N = 256) per instruction where possible
-                        const uint64_t db = umma_desc_k128(sbase + (bslot0 + (uint32_t)u) * kGramTile);
+                        const uint64_t db = umma_desc_k128(sbase + (uint32_t)(1 + u) * kGramTile);
                         const uint32_t idesc = (u + 1 < nu) ? kGramIdesc256 : kGramIdesc;
 #pragma unroll
                         for (int ks = 0; ks < 4; ++ks)         // K = 32 per instruction: +32 B in the atom
