@@ -161,3 +161,32 @@ def test_menger_full_size_structure(B, orc):
     m = sim.measure()
     assert 0 < int(m["n_up"][0]) < L ** 3
     sim.free()
+
+
+# ------------------------------------------------------------------ f-4 (part): L = 4096 on one GPU
+def test_L4096_one_gpu(B, orc):
+    """The size the paper hopes for next ("L=4096, in the near future"): 6.9e10 spins,
+    8 GiB packed (16 GiB with the ping-pong buffer).  fused2 == generic word for word, sampled
+    sites against the oracle's single-site evaluation, tensor == popcount measurement."""
+    L, seed = 4096, 12
+    a = B.Ising3D(L, [seed])
+    assert a.variant_name == "fused2" and a.measure_variant_name == "tensor"
+    xyz = _sample_sites(L, 3000, 23, RPT=60)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    got0 = _bits_at(a.get_state(buf), L, xyz)
+    assert np.array_equal(got0, orc.sites_after(seed, L, xyz, 0))
+    a.sweep(1)
+    got1 = _bits_at(a.get_state(buf), L, xyz)
+    assert np.array_equal(got1, orc.sites_after(seed, L, xyz, 2))
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_GENERIC)
+    b.sweep(1)
+    buf_b = np.empty(L ** 3 // 32, dtype=np.uint32)
+    assert np.array_equal(b.get_state(buf_b), buf)
+    b.free()
+    del buf_b
+    m_t = a.measure()
+    a.set_measure_variant(B.MEASURE_POPCOUNT)
+    m_p = a.measure()
+    assert np.array_equal(m_t["antipar"], m_p["antipar"]) and np.array_equal(m_t["n_up"], m_p["n_up"])
+    assert int(m_t["n_broken"][0]) == int(m_t["antipar"][0][:, 1].sum())
+    a.free()
