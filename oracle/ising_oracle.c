@@ -37,6 +37,10 @@
  *                         big-integer Python Philox
  *   orc_menger_solid / orc_init_menger : solid counts 20^k, the k = 1 cross written
  *                         out, self-similarity, tile-sign statistics, k = 0 iid
+ *   orc_corr_direct / orc_radial_bin / orc_radial_sums : P(0) = N, sum_d P(d) = M^2,
+ *                         P along the axes = N - 2 A_mu(r) (orc_measure), slab closed form,
+ *                         shell counts against a set-based Python count, bins vs exact
+ *                         rational comparison
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -316,6 +320,70 @@ void orc_init_menger(orc_t *o, int k)
                 o->s[orc_idx(o, x, y, z)] = (int8_t)(solid ? sign : -sign);
             }
     o->sweep = 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* The paper's own estimator:      */
+/* "C(r,t) shown in the main text is then obtained by radially          */
+/* averaging over the three-dimensional correlation matrix" with the    */
+/* matrix  [F^-1(|F s|^2)]_k = N * mean_i s_i s_{i+k}  (eq. 7).          */
+/* Here the matrix is written from its definition, as the INTEGER       */
+/*     P(d) = sum_i s_i s_{i+d},   d in [0,L)^3, periodic,               */
+/* by direct double loops (O(N^2): tiny L only; for larger L the Python  */
+/* wrapper takes the FFT route of eq. (7) in fp64 and rounds to the      */
+/* integer, pinned against this function).                               */
+/* Reading D12 (the paper does not define the radial average): the       */
+/* displacement d is folded to the minimal image, each component in      */
+/* (-L/2, L/2]; its bin is the integer b nearest to |d|, decided in      */
+/* integers: (2b-1)^2 <= 4|d|^2 < (2b+1)^2; bins b = 0..L/2 are kept     */
+/* (complete shells).  C_rad(b) = sum_{d in bin b} P(d) / (N * n(b))     */
+/* - m^2, n(b) = number of displacements in the bin.                     */
+/* ------------------------------------------------------------------ */
+int orc_radial_bin(int L, int dx, int dy, int dz)
+{
+    /* fold to the minimal image, components in (-L/2, L/2] */
+    if (dx > L / 2) dx -= L;
+    if (dy > L / 2) dy -= L;
+    if (dz > L / 2) dz -= L;
+    int64_t n4 = 4 * ((int64_t)dx * dx + (int64_t)dy * dy + (int64_t)dz * dz);
+    int64_t b = 0;
+    while ((2 * b + 1) * (2 * b + 1) <= n4) ++b;       /* first b with 4|d|^2 < (2b+1)^2 */
+    return (int)b;
+}
+
+/* P(d) for every d, direct definition.  out[(dz*L + dy)*L + dx], int64. */
+void orc_corr_direct(const orc_t *o, int64_t *out)
+{
+    const int L = o->L;
+    #pragma omp parallel for schedule(static)
+    for (int dz = 0; dz < L; ++dz)
+        for (int dy = 0; dy < L; ++dy)
+            for (int dx = 0; dx < L; ++dx) {
+                int64_t acc = 0;
+                for (int z = 0; z < L; ++z)
+                    for (int y = 0; y < L; ++y)
+                        for (int x = 0; x < L; ++x)
+                            acc += (int64_t)o->s[orc_idx(o, x, y, z)] *
+                                   (int64_t)o->s[orc_idx(o, orc_mod(x + dx, L), orc_mod(y + dy, L),
+                                                         orc_mod(z + dz, L))];
+                out[((size_t)dz * L + dy) * L + dx] = acc;
+            }
+}
+
+/* Radial sums of an integer field f[(dz*L + dy)*L + dx] over the bins of D12:
+ * sum[b] = sum of f over bin b, cnt[b] = n(b), b = 0..L/2. */
+void orc_radial_sums(int L, const int64_t *f, int64_t *sum, uint64_t *cnt)
+{
+    for (int b = 0; b <= L / 2; ++b) { sum[b] = 0; cnt[b] = 0; }
+    for (int dz = 0; dz < L; ++dz)
+        for (int dy = 0; dy < L; ++dy)
+            for (int dx = 0; dx < L; ++dx) {
+                int b = orc_radial_bin(L, dx, dy, dz);
+                if (b <= L / 2) {
+                    sum[b] += f[((size_t)dz * L + dy) * L + dx];
+                    cnt[b] += 1;
+                }
+            }
 }
 
 /* ------------------------------------------------------------------ */

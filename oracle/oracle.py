@@ -96,6 +96,13 @@ def lib():
         l.orc_menger_solid.restype = C.c_int
         l.orc_init_menger.argtypes = [C.c_void_p, C.c_int]
         l.orc_init_menger.restype = None
+        i64p = C.POINTER(C.c_int64)
+        l.orc_radial_bin.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
+        l.orc_radial_bin.restype = C.c_int
+        l.orc_corr_direct.argtypes = [C.c_void_p, i64p]
+        l.orc_corr_direct.restype = None
+        l.orc_radial_sums.argtypes = [C.c_int, i64p, i64p, u64p]
+        l.orc_radial_sums.restype = None
         l.orc_num_threads.argtypes = []
         l.orc_num_threads.restype = C.c_int
         l.orc_set_num_threads.argtypes = [C.c_int]
@@ -141,6 +148,21 @@ def menger_solid(u: int, v: int, w: int, k: int) -> int:
     return int(lib().orc_menger_solid(int(u), int(v), int(w), int(k)))
 
 
+def radial_bin(L: int, dx: int, dy: int, dz: int) -> int:
+    """D12: bin of the displacement (dx,dy,dz) in [0,L)^3 (minimal image, nearest integer to |d|)."""
+    return int(lib().orc_radial_bin(int(L), int(dx), int(dy), int(dz)))
+
+
+def radial_sums(L: int, field: np.ndarray):
+    """Sums of an int64 field[dz][dy][dx] over the radial bins 0..L/2 and the bin populations."""
+    f = np.ascontiguousarray(field, dtype=np.int64)
+    assert f.shape == (L, L, L)
+    s = np.zeros(L // 2 + 1, dtype=np.int64)
+    n = np.zeros(L // 2 + 1, dtype=np.uint64)
+    lib().orc_radial_sums(int(L), _p(f, C.c_int64), _p(s, C.c_int64), _p(n, C.c_uint64))
+    return s, n
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())
 
@@ -159,6 +181,17 @@ def postprocess(L, n_up, antipar, c_intercept=0.5):
     lib().orc_postprocess(L, int(n_up), _p(a, C.c_uint64), float(c_intercept),
                           C.byref(m), _p(Cr, C.c_double), C.byref(ell))
     return m.value, Cr, ell.value
+
+
+def _bins_numpy(L: int) -> np.ndarray:
+    """D12 bins of all displacements [dz][dy][dx], vectorised (same integer rule as orc_radial_bin)."""
+    d = np.arange(L, dtype=np.int64)
+    d = np.where(d > L // 2, d - L, d)
+    n4 = 4 * (d[:, None, None] ** 2 + d[None, :, None] ** 2 + d[None, None, :] ** 2)
+    b = np.floor((np.sqrt(n4.astype(np.float64)) + 1.0) / 2.0).astype(np.int64)
+    b = np.where((2 * b + 1) ** 2 <= n4, b + 1, b)          # integer fix-up of the float guess
+    b = np.where((b > 0) & ((2 * b - 1) ** 2 > n4), b - 1, b)
+    return b
 
 
 class Oracle:
@@ -215,6 +248,51 @@ class Oracle:
 
     def sweep(self, n: int = 1):
         self._l.orc_sweep(self._h, int(n))
+
+    # -- the paper's estimator: full correlation matrix + radial average (8(f)-1, D12) --------
+    def corr_direct(self) -> np.ndarray:
+        """P(d) = sum_i s_i s_{i+d} for every d, from the definition (O(N^2): L <= 32)."""
+        L = self.L
+        out = np.zeros((L, L, L), dtype=np.int64)
+        self._l.orc_corr_direct(self._h, _p(out, C.c_int64))
+        return out
+
+    def corr_fft(self) -> np.ndarray:
+        """The same integers by eq. (7): F^-1(|F s|^2) in fp64 (numpy), rounded to
+        the nearest integer (the error of the fp64 transforms is < 1e-3 for L <= 512)."""
+        s = self.spins.astype(np.float64)
+        p = np.fft.irfftn(np.abs(np.fft.rfftn(s)) ** 2, s=s.shape, axes=(0, 1, 2))
+        return np.rint(p).astype(np.int64)
+
+    def power_spectrum(self) -> np.ndarray:
+        """|F s|^2 on the full k grid [kz][ky][kx] (fp64)."""
+        return np.abs(np.fft.fftn(self.spins.astype(np.float64))) ** 2
+
+    def measure_radial(self, c_intercept: float = 0.5, direct: bool = False):
+        """D12: radially averaged C(r) (eq. (2) with the paper's estimator), shell populations,
+        radially averaged structure factor S(k) = |F s|^2 / N over the same bins in index space,
+        and ell from C_rad = c (D9 interpolation rule)."""
+        L = self.L
+        N = L ** 3
+        P = self.corr_direct() if direct else self.corr_fft()
+        sums, cnt = radial_sums(L, P)
+        m = float(self.spins.astype(np.int64).sum()) / N
+        C_rad = sums.astype(np.float64) / (float(N) * cnt.astype(np.float64)) - m * m
+        ps = self.power_spectrum()
+        nb = L // 2 + 1
+        S_sum = np.zeros(nb)
+        idx = np.arange(L)
+        bins = np.array([[[radial_bin(L, int(a), int(b), int(c)) for a in idx] for b in idx] for c in idx]) \
+            if L <= 16 else _bins_numpy(L)
+        for b in range(nb):
+            S_sum[b] = ps[bins == b].sum()
+        S_rad = S_sum / (float(N) * cnt.astype(np.float64))
+        ell = float("nan")
+        for r in range(nb - 1):
+            if C_rad[r] >= c_intercept and C_rad[r + 1] < c_intercept:
+                ell = r + (C_rad[r] - c_intercept) / (C_rad[r] - C_rad[r + 1])
+                break
+        return {"corr_sum": sums, "shell": cnt, "C_rad": C_rad, "S_rad": S_rad, "ell": ell, "m": m}
 
     def sweep_mixed(self, n: int = 1):
         """n sweeps of the mixed cycle (D10): the first colour is drawn per sweep."""

@@ -170,3 +170,105 @@ def test_init_menger_tile_signs_fair():
     # magnetisation of a sponge start: |m| per tile = (20 - 7)/27
     tiles = o.spins.reshape(32, 3, 32, 3, 32, 3).sum(axis=(1, 3, 5))
     assert set(np.unique(tiles)) <= {13, -13}
+
+
+# ------------------------------------------------------------------ f-1: FFT correlation + radial average
+def _exact_bin(L, dx, dy, dz):
+    """D12 restated with exact rationals: nearest integer to |d| of the minimal image."""
+    from fractions import Fraction
+    f = lambda v: v - L if v > L // 2 else v
+    n = f(dx) ** 2 + f(dy) ** 2 + f(dz) ** 2
+    b = 0
+    while Fraction(2 * b + 1, 2) ** 2 <= n:
+        b += 1
+    return b
+
+
+def test_radial_bins_and_shell_counts():
+    L = 12
+    seen = {}
+    for dz in range(L):
+        for dy in range(L):
+            for dx in range(L):
+                b = orc.radial_bin(L, dx, dy, dz)
+                assert b == _exact_bin(L, dx, dy, dz)
+                seen[b] = seen.get(b, 0) + 1
+    assert orc.radial_bin(L, 0, 0, 0) == 0 and seen[0] == 1
+    assert seen[1] == 6 + 12                      # |d| = 1 (6) and sqrt(2) = 1.41 (12); sqrt(3) -> 2
+    assert orc.radial_bin(L, L - 1, 0, 0) == 1 and orc.radial_bin(L, L // 2, 0, 0) == L // 2
+    _, cnt = orc.radial_sums(L, np.ones((L, L, L), dtype=np.int64))
+    assert [int(c) for c in cnt] == [seen.get(b, 0) for b in range(L // 2 + 1)]
+    # vectorised bins used by the FFT route == the C rule
+    from oracle.oracle import _bins_numpy
+    bn = _bins_numpy(L)
+    assert all(bn[z, y, x] == orc.radial_bin(L, x, y, z) for x in range(L) for y in range(L) for z in range(L))
+
+
+def test_correlation_matrix_identities():
+    """P(d) = sum_i s_i s_{i+d} from the definition: P(0) = N; sum_d P(d) = M^2; P(-d) = P(d);
+    along the axes P(r e_mu) = N - 2 A_mu(r) with A_mu from the (separately pinned) pair counts;
+    and the FFT route of eq. (7) gives the same integers."""
+    L = 8
+    o = orc.Oracle(L, 21)
+    o.sweep(3)
+    P = o.corr_direct()
+    N = L ** 3
+    M = int(o.spins.astype(np.int64).sum())
+    assert P[0, 0, 0] == N and P.sum() == M * M
+    assert np.array_equal(P, P[(-np.arange(L)) % L][:, (-np.arange(L)) % L][:, :, (-np.arange(L)) % L])
+    n_up, a = o.measure()
+    for r in range(L // 2 + 1):
+        assert P[0, 0, r] == N - 2 * int(a[0][r]) and P[0, r, 0] == N - 2 * int(a[1][r]) \
+            and P[r, 0, 0] == N - 2 * int(a[2][r])
+    assert np.array_equal(o.corr_fft(), P)
+    o16 = orc.Oracle(16, 5)
+    o16.sweep(2)
+    assert np.array_equal(o16.corr_fft(), o16.corr_direct())
+
+
+def test_correlation_closed_forms():
+    """All up: P = N everywhere, C_rad = 0.  Slab of thickness L/2 along z: P(d) depends on dz
+    only, P = N (1 - 4|dz|/L) for the folded dz (triangle wave)."""
+    L = 8
+    N = L ** 3
+    o = orc.Oracle(L, 1, init=False)
+    o.spins[...] = 1
+    r = o.measure_radial(direct=True)
+    assert np.all(r["corr_sum"] == N * r["shell"].astype(np.int64)) and np.allclose(r["C_rad"], 0.0)
+    o.spins[...] = inputs.slab(L, 2, 1, L // 2)
+    P = o.corr_direct()
+    for dz in range(L):
+        f = dz if dz <= L // 2 else L - dz
+        assert np.all(P[dz] == N - 4 * f * L * L)
+    assert o.measure_radial(direct=True)["m"] == 0.0
+
+
+def test_structure_factor_identities():
+    """S(k) = |F s|^2 / N: Parseval sum_k |F s|^2 = N * sum_i s_i^2 = N^2; the k = 0 bin is N m^2;
+    a plane wave s = sign(cos) along x puts all weight on kx = +-1 (odd harmonics), none on ky, kz != 0."""
+    L = 16
+    N = L ** 3
+    o = orc.Oracle(L, 8)
+    o.sweep(4)
+    ps = o.power_spectrum()
+    assert abs(ps.sum() - float(N) ** 2) < 1e-6 * N ** 2
+    r = o.measure_radial()
+    assert abs(r["S_rad"][0] - N * r["m"] ** 2) < 1e-9 * max(1.0, N * r["m"] ** 2)
+    o.spins[...] = inputs.slab(L, 0, 0, L // 2)           # +1 for x < L/2: a square wave along x
+    ps = o.power_spectrum()
+    assert np.all(ps[1:, :, :] < 1e-9) and np.all(ps[:, 1:, :] < 1e-9)
+    assert ps[0, 0, 1] > 0.3 * N ** 2 and abs(ps[0, 0, 2]) < 1e-9
+
+
+def test_radial_measure_fft_equals_direct_and_ell():
+    L = 16
+    o = orc.Oracle(L, 13)
+    o.sweep(6)
+    a = o.measure_radial(direct=True)
+    b = o.measure_radial(direct=False)
+    assert np.array_equal(a["corr_sum"], b["corr_sum"]) and np.array_equal(a["shell"], b["shell"])
+    assert a["C_rad"][0] == pytest.approx(1.0 - a["m"] ** 2, abs=1e-15)     # P(0) = N
+    # ell: first crossing of C_rad with c, linear interpolation (D9 rule)
+    C = a["C_rad"]
+    r0 = next(r for r in range(L // 2) if C[r] >= 0.5 > C[r + 1])
+    assert a["ell"] == pytest.approx(r0 + (C[r0] - 0.5) / (C[r0] - C[r0 + 1]), rel=1e-15)
