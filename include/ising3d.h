@@ -193,6 +193,35 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);
 int ising3d_measure(ising3d_t *h, ising3d_meas_t *out);
 
 /*
+ * The paper's own estimator: the full correlation matrix by eq. (7)
+ * PAPER.md:128, mean_i s_i s_{i+k} = [F^-1(|F s|^2)]_k (3-D real-data DFT in place, fp64, cuFFT),
+ * then "radially averaging over the three-dimensional correlation matrix", and
+ * the structure factor S(k) = |F s|^2 / N.  Reading D12: displacements are folded to
+ * the minimal image (components in (-L/2, L/2]) and binned by the integer nearest to |d|
+ * ((2b-1)^2 <= 4|d|^2 < (2b+1)^2), bins b = 0..L/2; the same bins in index space for k.
+ * The transform of +-1 data is an integer up to round-off, so P(d) = sum_i s_i s_{i+d} is
+ * recovered exactly (llrint) and corr_sum holds exact integer sums.
+ *   corr_sum [n_rep][L/2+1]  HOST  sum of P(d) over bin b
+ *   shell    [L/2+1]         HOST  number of displacements in bin b
+ *   C_rad    [n_rep][L/2+1]  HOST  corr_sum / (N * shell) - m^2            (eq. 2)
+ *   S_rad    [n_rep][L/2+1]  HOST  may be NULL; mean of |F s|^2 / N over the k bin
+ *   ell      [n_rep]         HOST  may be NULL; first C_rad = c_intercept crossing (D9 rule)
+ * Needs 8 bytes per site of device memory plus the cuFFT work area, allocated by the library
+ * on first use (ENOMEM if that fails; the handle stays usable).  Synchronises the stream.
+ */
+typedef struct {
+    int32_t   L, n_rep;
+    uint64_t  sweep;
+    int64_t  *corr_sum;
+    uint64_t *shell;
+    double   *C_rad;
+    double   *S_rad;
+    double   *ell;
+    double    c_intercept;
+} ising3d_radial_t;
+int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out);
+
+/*
  * Copy the canonical packed state (D3) to / from HOST memory.
  * n_words must equal n_rep * L^3/32.  Both synchronise the stream.
  * set_state also sets the sweep counter (the next sweep executed has index

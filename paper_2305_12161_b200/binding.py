@@ -25,7 +25,7 @@ EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
     "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_init_menger", "ising3d_set_measure_variant",
     "ising3d_measure_variant_name",
-    "ising3d_sweep", "ising3d_measure", "ising3d_get_state", "ising3d_set_state",
+    "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
     "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size", "ising3d_sync",
     "ising3d_free", "ising3d_last_error",
@@ -42,6 +42,13 @@ class MeasT(C.Structure):
     _fields_ = [("L", C.c_int32), ("n_rep", C.c_int32), ("sweep", C.c_uint64),
                 ("n_up", C.POINTER(C.c_uint64)), ("n_broken", C.POINTER(C.c_uint64)),
                 ("antipar", C.POINTER(C.c_uint64)), ("C", C.POINTER(C.c_double)),
+                ("ell", C.POINTER(C.c_double)), ("c_intercept", C.c_double)]
+
+
+class RadialT(C.Structure):
+    _fields_ = [("L", C.c_int32), ("n_rep", C.c_int32), ("sweep", C.c_uint64),
+                ("corr_sum", C.POINTER(C.c_int64)), ("shell", C.POINTER(C.c_uint64)),
+                ("C_rad", C.POINTER(C.c_double)), ("S_rad", C.POINTER(C.c_double)),
                 ("ell", C.POINTER(C.c_double)), ("c_intercept", C.c_double)]
 
 
@@ -74,6 +81,7 @@ def load():
         "ising3d_init_menger": (C.c_int, [vp, C.c_int]),
         "ising3d_sweep": (C.c_int, [vp, u64]),
         "ising3d_measure": (C.c_int, [vp, C.POINTER(MeasT)]),
+        "ising3d_measure_radial": (C.c_int, [vp, C.POINTER(RadialT)]),
         "ising3d_get_state": (C.c_int, [vp, vp, C.c_size_t, u64p]),
         "ising3d_set_state": (C.c_int, [vp, vp, C.c_size_t, u64]),
         "ising3d_get_state_device": (C.c_int, [vp, vp, C.c_size_t, u64p]),
@@ -226,6 +234,20 @@ class Ising3D:
         _check(self._l.ising3d_measure(self._h, C.byref(m)))
         return {"sweep": int(m.sweep), "n_up": n_up, "n_broken": n_broken, "antipar": antipar,
                 "C": Cr, "ell": ell}
+
+    def measure_radial(self, c_intercept: float = 0.5):
+        nb = self.L // 2 + 1
+        corr = np.zeros((self.n_rep, nb), dtype=np.int64)
+        shell = np.zeros(nb, dtype=np.uint64)
+        Cr = np.zeros((self.n_rep, nb), dtype=np.float64)
+        Sr = np.zeros((self.n_rep, nb), dtype=np.float64)
+        ell = np.zeros(self.n_rep, dtype=np.float64)
+        m = RadialT(self.L, self.n_rep, 0, corr.ctypes.data_as(C.POINTER(C.c_int64)),
+                    shell.ctypes.data_as(C.POINTER(C.c_uint64)), Cr.ctypes.data_as(C.POINTER(C.c_double)),
+                    Sr.ctypes.data_as(C.POINTER(C.c_double)), ell.ctypes.data_as(C.POINTER(C.c_double)),
+                    float(c_intercept))
+        _check(self._l.ising3d_measure_radial(self._h, C.byref(m)))
+        return {"sweep": int(m.sweep), "corr_sum": corr, "shell": shell, "C_rad": Cr, "S_rad": Sr, "ell": ell}
 
     def get_state(self, out: np.ndarray | None = None) -> np.ndarray:
         n = self.n_rep * self.L ** 3 // 32

@@ -14,6 +14,7 @@ NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared",
     "-Xptxas", "-v",
+    "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64",
 ]
 
 

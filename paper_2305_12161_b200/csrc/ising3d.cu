@@ -12,10 +12,12 @@
 #include <vector>
 
 #include <cuda_runtime.h>
+#include <cufft.h>
 
 #include "kernels_fused.cuh"
 #include "kernels_fused2.cuh"
 #include "kernels_generic.cuh"
+#include "kernels_fft.cuh"
 #include "kernels_gram.cuh"
 #include "kernels_measure.cuh"
 #include "kernels_resident.cuh"
@@ -61,6 +63,12 @@ struct ising3d {
     int measure_variant = ISING3D_MEASURE_AUTO;
     unsigned long long *d_gsum = nullptr;      // [n_rep][3][L/2+1] Gram diagonal sums
     unsigned int *d_queue = nullptr;           // [3 n_rep] task counters of gram_kernel
+    // FFT estimator (ising3d_measure_radial): created on first use, library-owned
+    double *fft_buf = nullptr;                 // [L][L][L+2] in-place real / half-complex field
+    void *fft_work = nullptr;                  // cuFFT work area shared by both plans
+    unsigned long long *d_rad = nullptr;       // [2][L/2+1] P sums, shell counts; then [L/2+1] doubles
+    cufftHandle plan_fwd = 0, plan_inv = 0;
+    bool fft_ready = false;
     uint64_t launches = 0;
     int sm_count = 148;
     mutable ising::ResidentPlan res_plan = {0, 0};
@@ -273,6 +281,52 @@ void postprocess(int L, uint64_t n_up, const uint64_t *antipar, double c_interce
                 break;
             }
     }
+}
+
+// cuFFT plans and buffers of the radial estimator, on first use (8 bytes per site + work area)
+int fft_setup(ising3d *h)
+{
+    if (h->fft_ready) return ISING3D_OK;
+    const int L = h->L, H = L / 2 + 1;
+    const size_t buf_bytes = (size_t)L * L * (L + 2) * sizeof(double);
+    auto cleanup = [&]() {
+        if (h->plan_fwd) cufftDestroy(h->plan_fwd);
+        if (h->plan_inv) cufftDestroy(h->plan_inv);
+        if (h->fft_buf) cudaFree(h->fft_buf);
+        if (h->fft_work) cudaFree(h->fft_work);
+        if (h->d_rad) cudaFree(h->d_rad);
+        h->plan_fwd = h->plan_inv = 0;
+        h->fft_buf = nullptr;
+        h->fft_work = nullptr;
+        h->d_rad = nullptr;
+        cudaGetLastError();
+    };
+    size_t ws_f = 0, ws_i = 0;
+    if (cudaMalloc(&h->fft_buf, buf_bytes) != cudaSuccess ||
+        cudaMalloc(&h->d_rad, (size_t)3 * H * 8) != cudaSuccess) {
+        cleanup();
+        return fail(ISING3D_ENOMEM, "radial estimator: cannot allocate the 8 bytes/site FFT field");
+    }
+    if (cufftCreate(&h->plan_fwd) != CUFFT_SUCCESS || cufftCreate(&h->plan_inv) != CUFFT_SUCCESS ||
+        cufftSetAutoAllocation(h->plan_fwd, 0) != CUFFT_SUCCESS ||
+        cufftSetAutoAllocation(h->plan_inv, 0) != CUFFT_SUCCESS ||
+        cufftMakePlan3d(h->plan_fwd, L, L, L, CUFFT_D2Z, &ws_f) != CUFFT_SUCCESS ||
+        cufftMakePlan3d(h->plan_inv, L, L, L, CUFFT_Z2D, &ws_i) != CUFFT_SUCCESS) {
+        cleanup();
+        return fail(ISING3D_ECUDA, "radial estimator: cuFFT plan creation failed");
+    }
+    const size_t ws = std::max(ws_f, ws_i);
+    if (ws && cudaMalloc(&h->fft_work, ws) != cudaSuccess) {
+        cleanup();
+        return fail(ISING3D_ENOMEM, "radial estimator: cannot allocate the cuFFT work area");
+    }
+    if (cufftSetWorkArea(h->plan_fwd, h->fft_work) != CUFFT_SUCCESS ||
+        cufftSetWorkArea(h->plan_inv, h->fft_work) != CUFFT_SUCCESS) {
+        cleanup();
+        return fail(ISING3D_ECUDA, "radial estimator: cufftSetWorkArea failed");
+    }
+    h->fft_ready = true;
+    return ISING3D_OK;
 }
 
 // A_mu(r) on the tensor cores (kernels_gram.cuh): per replica and axis, gather the line words
@@ -502,6 +556,69 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
     return ISING3D_OK;
 }
 
+int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out)
+{
+    if (!h || !out) return fail(ISING3D_EINVAL, "null pointer");
+    if (out->L != h->L || out->n_rep != h->n_rep)
+        return fail(ISING3D_EINVAL, "measurement record shape does not match the handle");
+    if (!out->corr_sum || !out->shell || !out->C_rad)
+        return fail(ISING3D_EINVAL, "corr_sum, shell and C_rad must be provided");
+    const int rc = fft_setup(h);
+    if (rc != ISING3D_OK) return rc;
+    const int L = h->L, H = L / 2 + 1, cpr = h->counts_per_replica();
+    const double N = (double)L * L * L;
+    if (cufftSetStream(h->plan_fwd, h->stream) != CUFFT_SUCCESS ||
+        cufftSetStream(h->plan_inv, h->stream) != CUFFT_SUCCESS)
+        return fail(ISING3D_ECUDA, "cufftSetStream failed");
+    std::vector<unsigned long long> host((size_t)3 * H);
+    const int grid = h->sm_count * 8;
+    out->sweep = h->sweep;
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        const uint32_t *st = h->state[h->cur] + (size_t)rep * h->words_per_replica();
+        unsigned long long *d_cnt = h->d_counts + (size_t)rep * cpr;
+        CUDA_TRY(cudaMemsetAsync(d_cnt, 0, 8, h->stream));
+        CUDA_TRY(cudaMemsetAsync(h->d_rad, 0, (size_t)3 * H * 8, h->stream));
+        ising::count_up_kernel<<<dim3((unsigned)grid, 1), 256, 0, h->stream>>>(st, d_cnt, h->words_per_replica(), cpr);
+        ising::unpack_real_kernel<<<grid, 256, 0, h->stream>>>(st, h->fft_buf, L);
+        if (cufftExecD2Z(h->plan_fwd, h->fft_buf, reinterpret_cast<cufftDoubleComplex *>(h->fft_buf)) != CUFFT_SUCCESS)
+            return fail(ISING3D_ECUDA, "cufftExecD2Z failed");
+        ising::power_kernel<<<grid, 256, (size_t)H * 8, h->stream>>>(
+            reinterpret_cast<double2 *>(h->fft_buf), reinterpret_cast<double *>(h->d_rad + 2 * H), L);
+        if (cufftExecZ2D(h->plan_inv, reinterpret_cast<cufftDoubleComplex *>(h->fft_buf), h->fft_buf) != CUFFT_SUCCESS)
+            return fail(ISING3D_ECUDA, "cufftExecZ2D failed");
+        ising::radial_kernel<<<grid, 256, (size_t)2 * H * 8, h->stream>>>(h->fft_buf, h->d_rad, h->d_rad + H, L);
+        h->launches += 4;
+        CUDA_TRY(cudaGetLastError());
+        unsigned long long n_up = 0;
+        CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_rad, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(&n_up, d_cnt, 8, cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        // D12 / D9 post-processing in fp64, this order
+        const double m = (double)(2 * (int64_t)n_up - (int64_t)N) / N;
+        double *C = out->C_rad + (size_t)rep * H;
+        for (int b = 0; b < H; ++b) {
+            const int64_t ps = (int64_t)host[b];
+            out->corr_sum[(size_t)rep * H + b] = ps;
+            out->shell[b] = host[H + b];
+            C[b] = (double)ps / (N * (double)host[H + b]) - m * m;
+            if (out->S_rad) {
+                double sv;
+                std::memcpy(&sv, &host[2 * H + b], 8);
+                out->S_rad[(size_t)rep * H + b] = sv / (N * (double)host[H + b]);
+            }
+        }
+        if (out->ell) {
+            out->ell[rep] = std::nan("");
+            for (int b = 0; b + 1 < H; ++b)
+                if (C[b] >= out->c_intercept && C[b + 1] < out->c_intercept) {
+                    out->ell[rep] = (double)b + (C[b] - out->c_intercept) / (C[b] - C[b + 1]);
+                    break;
+                }
+        }
+    }
+    return ISING3D_OK;
+}
+
 int ising3d_get_state(ising3d_t *h, uint32_t *words, size_t n_words, uint64_t *sweep)
 {
     if (!h || !words) return fail(ISING3D_EINVAL, "null pointer");
@@ -580,6 +697,11 @@ void ising3d_free(ising3d_t *h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
+    if (h->plan_fwd) cufftDestroy(h->plan_fwd);
+    if (h->plan_inv) cufftDestroy(h->plan_inv);
+    if (h->fft_buf) cudaFree(h->fft_buf);
+    if (h->fft_work) cudaFree(h->fft_work);
+    if (h->d_rad) cudaFree(h->d_rad);
     if (h->owns_mem && h->base) cudaFree(h->base);
     delete h;
 }

@@ -190,3 +190,69 @@ def test_L4096_one_gpu(B, orc):
     assert np.array_equal(m_t["antipar"], m_p["antipar"]) and np.array_equal(m_t["n_up"], m_p["n_up"])
     assert int(m_t["n_broken"][0]) == int(m_t["antipar"][0][:, 1].sum())
     a.free()
+
+
+# ------------------------------------------------------------------ f-1: FFT correlation + radial average
+def _check_radial(got, want, rep=0):
+    assert np.array_equal(got["corr_sum"][rep], want["corr_sum"])          # exact integers
+    assert np.array_equal(got["shell"], want["shell"])
+    assert np.all(np.abs(got["C_rad"][rep] - want["C_rad"]) <= 1e-12 * np.maximum(1.0, np.abs(want["C_rad"])))
+    # S(k): fp64 sums in a different order; D12 tolerance 1e-9 of the largest bin
+    scale = np.abs(want["S_rad"]).max()
+    assert np.all(np.abs(got["S_rad"][rep] - want["S_rad"]) <= 1e-9 * scale)
+    if np.isnan(want["ell"]):
+        assert np.isnan(got["ell"][rep])
+    else:
+        assert abs(got["ell"][rep] - want["ell"]) <= 1e-12 * abs(want["ell"])
+
+
+@pytest.mark.parametrize("L,seed,sweeps", [(64, 1, 0), (64, 1, 12), (128, 7, 5), (192, 8, 3), (256, 2, 20)])
+def test_radial_estimator_against_oracle(B, orc, L, seed, sweeps):
+    sim = B.Ising3D(L, [seed])
+    ref = orc.Oracle(L, seed)
+    sim.sweep(sweeps)
+    ref.sweep(sweeps)
+    _check_radial(sim.measure_radial(), ref.measure_radial())
+    # measuring does not disturb the state or the other measurement
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+
+
+def test_radial_estimator_batch_and_structured(B, orc):
+    L, seeds = 64, [100, 101, 102]
+    batch = B.Ising3D(L, seeds)
+    batch.sweep(4)
+    got = batch.measure_radial(c_intercept=0.3)
+    for i, s in enumerate(seeds):
+        ref = orc.Oracle(L, s)
+        ref.sweep(4)
+        _check_radial(got, ref.measure_radial(c_intercept=0.3), rep=i)
+    batch.free()
+    sim = B.Ising3D(L, [1])
+    ref = orc.Oracle(L, 1, init=False)
+    for s0 in (inputs.all_up(L), inputs.slab(L, 2, 5, L // 2), inputs.neel(L)):
+        w = inputs.pack_spins(s0)
+        sim.set_state(w, 0)
+        ref.import_words(w, 0)
+        _check_radial(sim.measure_radial(), ref.measure_radial())
+    sim.free()
+
+
+def test_radial_estimator_large_identities(B):
+    """L = 1024 (8.6 GB field): what holds at any size -- P(0) = N in bin 0, S(k = 0) = N m^2,
+    Parseval through the bins that are complete, C_rad(0) = 1 - m^2."""
+    L = 1024
+    sim = B.Ising3D(L, [3])
+    sim.sweep(10)
+    r = sim.measure_radial()
+    m = sim.measure()
+    N = L ** 3
+    mag = (2.0 * float(m["n_up"][0]) - N) / N
+    assert int(r["corr_sum"][0][0]) == N and int(r["shell"][0]) == 1 and int(r["shell"][1]) == 18
+    assert abs(r["C_rad"][0][0] - (1.0 - mag * mag)) < 1e-12
+    assert abs(r["S_rad"][0][0] - N * mag * mag) <= 1e-9 * max(1.0, N * mag * mag)
+    # the radial C and the axis-averaged C agree to a few per cent at short distance
+    assert abs(r["C_rad"][0][1] - m["C"][0][1]) < 0.1
+    assert abs(r["ell"][0] - m["ell"][0]) < 0.25 * m["ell"][0]
+    sim.free()
