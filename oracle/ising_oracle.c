@@ -41,6 +41,11 @@
  *                         P along the axes = N - 2 A_mu(r) (orc_measure), slab closed form,
  *                         shell counts against a set-based Python count, bins vs exact
  *                         rational comparison
+ *   orc_glauber_thresholds / orc_site_uniform / orc_sweep_T : p(6-n) = 1 - p(n), p(3) = 1/2,
+ *                         hand-computed thresholds, T -> infinity closed form (flip iff the top
+ *                         Philox plane bit is 0), acceptance frequencies on uniform-n states
+ *                         (all up: n = 0, Neel: n = 6) within binomial errors, T -> 0 limit of
+ *                         the deterministic moves, energy relaxation towards the T = 0 quench
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -320,6 +325,72 @@ void orc_init_menger(orc_t *o, int k)
                 o->s[orc_idx(o, x, y, z)] = (int8_t)(solid ? sign : -sign);
             }
     o->sweep = 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Finite-temperature Glauber dynamics (eq. (5)       */
+/* PAPER.md:101): a proposed flip is accepted with probability          */
+/*     p_acc(Delta E, T) = 1 / (1 + exp(Delta E / T)),   k_B = 1,        */
+/* Delta E = 2 s_i sum_nn s_j = 12 - 4n (n antiparallel neighbours).     */
+/* Reading D13 (the paper does not run T > 0 and names no RNG): each     */
+/* site draws a 32-bit uniform u per sweep, u = sum_j b_j 2^(31-j) with  */
+/* b_j the site's bit of Philox(key = seed, counter = (q, t, c, 4 + j)), */
+/* j = 0..31 (one Philox call yields bit j of u for the 128 spins of a   */
+/* group); the flip is accepted iff u < thr[n], thr[n] =                 */
+/* floor(p_acc(12 - 4n, T) * 2^32) as a 64-bit integer in [0, 2^32]      */
+/* (p = 1 always accepts), computed in fp64 with the C library's exp().  */
+/* Sweep order as at T = 0 (colour 0, then colour 1).                    */
+/* ------------------------------------------------------------------ */
+void orc_glauber_thresholds(double T, uint64_t thr[7])
+{
+    for (int n = 0; n <= 6; ++n) {
+        double dE = 12.0 - 4.0 * (double)n;
+        double p = 1.0 / (1.0 + exp(dE / T));
+        thr[n] = (uint64_t)floor(p * 4294967296.0);
+    }
+}
+
+uint32_t orc_site_uniform(uint64_t seed, int L, int x, int y, int z, uint32_t t)
+{
+    uint32_t u = 0;
+    for (uint32_t j = 0; j < 32; ++j)
+        u |= (uint32_t)orc_site_bit(seed, L, x, y, z, t, 4u + j) << (31u - j);
+    return u;
+}
+
+static inline void orc_update_site_T(orc_t *o, int x, int y, int z, uint32_t t, const uint64_t thr[7])
+{
+    const int L = o->L;
+    int8_t *si = &o->s[orc_idx(o, x, y, z)];
+    int n = 0;                                   /* antiparallel neighbours */
+    n += o->s[orc_idx(o, orc_mod(x + 1, L), y, z)] != *si;
+    n += o->s[orc_idx(o, orc_mod(x - 1, L), y, z)] != *si;
+    n += o->s[orc_idx(o, x, orc_mod(y + 1, L), z)] != *si;
+    n += o->s[orc_idx(o, x, orc_mod(y - 1, L), z)] != *si;
+    n += o->s[orc_idx(o, x, y, orc_mod(z + 1, L))] != *si;
+    n += o->s[orc_idx(o, x, y, orc_mod(z - 1, L))] != *si;
+    if ((uint64_t)orc_site_uniform(o->seed, L, x, y, z, t) < thr[n]) *si = (int8_t)(-*si);
+}
+
+void orc_half_sweep_T(orc_t *o, uint32_t t, int c, const uint64_t thr[7])
+{
+    const int L = o->L;
+    #pragma omp parallel for schedule(static)
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x)
+                if (((x + y + z) & 1) == c) orc_update_site_T(o, x, y, z, t, thr);
+}
+
+void orc_sweep_T(orc_t *o, uint64_t n_sweeps, double T)
+{
+    uint64_t thr[7];
+    orc_glauber_thresholds(T, thr);
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        orc_half_sweep_T(o, o->sweep, 0, thr);
+        orc_half_sweep_T(o, o->sweep, 1, thr);
+        o->sweep += 1;
+    }
 }
 
 /* ------------------------------------------------------------------ */

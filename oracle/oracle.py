@@ -103,6 +103,14 @@ def lib():
         l.orc_corr_direct.restype = None
         l.orc_radial_sums.argtypes = [C.c_int, i64p, i64p, u64p]
         l.orc_radial_sums.restype = None
+        l.orc_glauber_thresholds.argtypes = [C.c_double, u64p]
+        l.orc_glauber_thresholds.restype = None
+        l.orc_site_uniform.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint32]
+        l.orc_site_uniform.restype = C.c_uint32
+        l.orc_sweep_T.argtypes = [C.c_void_p, C.c_uint64, C.c_double]
+        l.orc_sweep_T.restype = None
+        l.orc_half_sweep_T.argtypes = [C.c_void_p, C.c_uint32, C.c_int, u64p]
+        l.orc_half_sweep_T.restype = None
         l.orc_num_threads.argtypes = []
         l.orc_num_threads.restype = C.c_int
         l.orc_set_num_threads.argtypes = [C.c_int]
@@ -161,6 +169,18 @@ def radial_sums(L: int, field: np.ndarray):
     n = np.zeros(L // 2 + 1, dtype=np.uint64)
     lib().orc_radial_sums(int(L), _p(f, C.c_int64), _p(s, C.c_int64), _p(n, C.c_uint64))
     return s, n
+
+
+def glauber_thresholds(T: float) -> np.ndarray:
+    """D13: thr[n] = floor(2^32 / (1 + exp((12 - 4n)/T))), n = 0..6 antiparallel neighbours."""
+    thr = np.zeros(7, dtype=np.uint64)
+    lib().orc_glauber_thresholds(float(T), _p(thr, C.c_uint64))
+    return thr
+
+
+def site_uniform(seed: int, L: int, x: int, y: int, z: int, t: int) -> int:
+    """D13: the site's 32-bit uniform of sweep t (Philox bit planes, tags 4..35)."""
+    return int(lib().orc_site_uniform(int(seed), int(L), int(x), int(y), int(z), int(t)))
 
 
 def num_threads() -> int:
@@ -293,6 +313,14 @@ class Oracle:
                 ell = r + (C_rad[r] - c_intercept) / (C_rad[r] - C_rad[r + 1])
                 break
         return {"corr_sum": sums, "shell": cnt, "C_rad": C_rad, "S_rad": S_rad, "ell": ell, "m": m}
+
+    def sweep_T(self, n: int, T: float):
+        """n sweeps of finite-temperature Glauber dynamics (eq. (5), D13)."""
+        self._l.orc_sweep_T(self._h, int(n), float(T))
+
+    def half_sweep_T(self, t: int, c: int, T: float):
+        thr = glauber_thresholds(T)
+        self._l.orc_half_sweep_T(self._h, int(t), int(c), _p(thr, C.c_uint64))
 
     def sweep_mixed(self, n: int = 1):
         """n sweeps of the mixed cycle (D10): the first colour is drawn per sweep."""

@@ -272,3 +272,100 @@ def test_radial_measure_fft_equals_direct_and_ell():
     C = a["C_rad"]
     r0 = next(r for r in range(L // 2) if C[r] >= 0.5 > C[r + 1])
     assert a["ell"] == pytest.approx(r0 + (C[r0] - 0.5) / (C[r0] - C[r0 + 1]), rel=1e-15)
+
+
+# ------------------------------------------------------------------ f-4: finite-temperature Glauber
+def test_glauber_thresholds():
+    """eq. (5) PAPER.md:101 with Delta E = 12 - 4n: p(3) = 1/2 exactly, p(6-n) = 1 - p(n), hand
+    values at T = 4 (p(0) = 1/(1+e^3) = 0.0474258731...), limits T -> 0 (eq. (6)) and T -> inf."""
+    import math
+    thr = orc.glauber_thresholds(4.0)
+    assert int(thr[3]) == 2 ** 31
+    for n in range(7):
+        assert abs(int(thr[n]) + int(thr[6 - n]) - 2 ** 32) <= 1
+        want = 1.0 / (1.0 + math.exp((12 - 4 * n) / 4.0))
+        assert abs(int(thr[n]) / 2.0 ** 32 - want) < 2.0 ** -31
+    assert abs(int(thr[0]) / 2.0 ** 32 - 0.04742587317756678) < 1e-9
+    cold = orc.glauber_thresholds(0.05)
+    assert [int(v) for v in cold] == [0, 0, 0, 2 ** 31, 2 ** 32, 2 ** 32, 2 ** 32]     # eq. (6)
+    hot = orc.glauber_thresholds(1e12)
+    assert all(abs(int(v) - 2 ** 31) <= 1 for v in hot)
+
+
+def test_site_uniform_is_the_documented_bit_planes():
+    """D13: u = sum_j b_j 2^(31-j), b_j the site's bit of Philox(counter (q, t, c, 4 + j))."""
+    from test_oracle_pins import py_site_bit
+    L, seed = 8, 0x1234567899
+    for (x, y, z, t) in [(0, 0, 0, 0), (7, 3, 5, 2), (2, 6, 1, 1000)]:
+        want = 0
+        for j in range(32):
+            want |= py_site_bit(seed, L, x, y, z, t, 4 + j) << (31 - j)
+        assert orc.site_uniform(seed, L, x, y, z, t) == want
+    us = np.array([orc.site_uniform(3, 8, x, y, z, 0) for x in range(8) for y in range(8) for z in range(8)],
+                  dtype=np.float64) / 2.0 ** 32
+    assert abs(us.mean() - 0.5) < 4 * (1 / 12 ** 0.5) / 512 ** 0.5
+
+
+def test_glauber_acceptance_frequencies():
+    """States where every site has the same n: all up (n = 0) flips a fraction p(0) of the first
+    colour, the Neel state (n = 6) a fraction p(6) = 1 - p(0); binomial 4 sigma."""
+    import math
+    L, T = 32, 4.0
+    half = L ** 3 // 2
+    p0 = 1.0 / (1.0 + math.exp(12 / T))
+    o = orc.Oracle(L, 17, init=False)
+    o.spins[...] = 1
+    o.half_sweep_T(0, 0, T)
+    flipped = int((o.spins == -1).sum())
+    assert abs(flipped - half * p0) < 4 * math.sqrt(half * p0 * (1 - p0))
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    assert np.all(o.spins[((x + y + z) & 1) == 1] == 1)          # the other colour was not proposed
+    o.spins[...] = inputs.neel(L)
+    o.half_sweep_T(3, 0, T)
+    kept = int((o.spins[((x + y + z) & 1) == 0] == 1).sum())     # black sites that did NOT flip
+    assert abs(kept - half * p0) < 4 * math.sqrt(half * p0 * (1 - p0))
+
+
+def test_glauber_hot_limit_closed_form():
+    """T -> infinity: thr = 2^31 for every n, so a site flips iff the top bit of u (Philox tag 4)
+    is 0, whatever its neighbours."""
+    from test_oracle_pins import py_site_bit
+    L, seed = 6, 5
+    o = orc.Oracle(L, seed)
+    before = o.spins.copy()
+    o.half_sweep_T(0, 0, 1e12)
+    for z in range(L):
+        for y in range(L):
+            for x in range(L):
+                if (x + y + z) & 1:
+                    assert o.spins[z, y, x] == before[z, y, x]
+                else:
+                    flip = py_site_bit(seed, L, x, y, z, 0, 4) == 0
+                    assert o.spins[z, y, x] == (-before[z, y, x] if flip else before[z, y, x])
+
+
+def test_glauber_cold_limit_and_relaxation():
+    """T -> 0: the deterministic moves of eq. (6) (n >= 4 flips, n <= 2 stays) are reproduced;
+    at T = 1.5 the energy of a quench relaxes far below the random start and stays above the
+    ground state; sweep_T(n) == n x (half_sweep_T colour 0, colour 1)."""
+    L = 16
+    a = orc.Oracle(L, 9)
+    b = orc.Oracle(L, 9)
+    s0 = a.spins.copy()
+    a.half_sweep_T(0, 0, 0.05)
+    b.half_sweep(0, 0)                                           # T = 0 rule: same except at ties
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    nbr = sum(np.roll(s0, sh, axis=ax) for ax in (0, 1, 2) for sh in (1, -1))
+    n_anti = (6 - s0 * nbr) // 2
+    det = (((x + y + z) & 1) == 0) & (n_anti != 3)
+    assert np.array_equal(a.spins[det], b.spins[det])
+    c = orc.Oracle(L, 4)
+    d = orc.Oracle(L, 4)
+    e0 = c.measure([1])[1].sum()
+    c.sweep_T(12, 1.5)
+    for t in range(12):
+        d.half_sweep_T(t, 0, 1.5)
+        d.half_sweep_T(t, 1, 1.5)
+    assert np.array_equal(c.spins, d.spins) and c.sweep_count == 12
+    e1 = c.measure([1])[1].sum()
+    assert 0 < e1 < 0.45 * e0
