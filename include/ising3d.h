@@ -171,6 +171,19 @@ int ising3d_init_menger(ising3d_t *h, int k);
  */
 int ising3d_set_cycle(ising3d_t *h, int cycle);
 
+/*
+ * Temperature of the quench.  T = 0 (default): the paper's T -> 0 acceptance, eq. (6)
+ * PAPER.md:105-108 ("which is the acceptance probability we use throughout").  T > 0 (k_B = 1):
+ * the Glauber probability of eq. (5), p = 1 / (1 + exp(Delta E / T)) (the paper's
+ * announced follow-up).  Reading D13: a site with n antiparallel
+ * neighbours (Delta E = 12 - 4n) flips iff u < thr[n], thr[n] = floor(2^32 p) in [0, 2^32]
+ * (fp64), u = sum_j b_j 2^(31-j) its 32-bit uniform of the sweep, b_j the site's bit of
+ * Philox(key = seed, counter = (q, t, c, 4 + j)), j = 0..31.  Sweeps at T > 0 run the
+ * "glauber" kernel (two launches per sweep, any L, batches) whatever the sweep variant.
+ * EINVAL for negative or non-finite T.
+ */
+int ising3d_set_temperature(ising3d_t *h, double T);
+
 /* Use `cuda_stream` (a cudaStream_t owned by the caller) for all later work. */
 int ising3d_set_stream(ising3d_t *h, void *cuda_stream);
 

@@ -23,7 +23,7 @@ VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT =
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
-    "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_init_menger", "ising3d_set_measure_variant",
+    "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_set_temperature", "ising3d_init_menger", "ising3d_set_measure_variant",
     "ising3d_measure_variant_name",
     "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
@@ -76,6 +76,7 @@ def load():
         "ising3d_set_stream": (C.c_int, [vp, vp]),
         "ising3d_set_variant": (C.c_int, [vp, C.c_int]),
         "ising3d_set_cycle": (C.c_int, [vp, C.c_int]),
+        "ising3d_set_temperature": (C.c_int, [vp, C.c_double]),
         "ising3d_set_measure_variant": (C.c_int, [vp, C.c_int]),
         "ising3d_measure_variant_name": (C.c_char_p, [vp]),
         "ising3d_init_menger": (C.c_int, [vp, C.c_int]),
@@ -185,6 +186,9 @@ class Ising3D:
     @property
     def measure_variant_name(self) -> str:
         return self._l.ising3d_measure_variant_name(self._h).decode()
+
+    def set_temperature(self, T: float):
+        _check(self._l.ising3d_set_temperature(self._h, float(T)))
 
     def set_cycle(self, cycle: int):
         _check(self._l.ising3d_set_cycle(self._h, cycle))

@@ -61,6 +61,8 @@ struct ising3d {
     int variant = ISING3D_VARIANT_AUTO;
     int cycle = ISING3D_CYCLE_01;
     int measure_variant = ISING3D_MEASURE_AUTO;
+    double temperature = 0.0;                  // 0 = the paper's T -> 0 rule (eq. 6); > 0: eq. (5), D13
+    ising::GlauberTables glauber = {};
     unsigned long long *d_gsum = nullptr;      // [n_rep][3][L/2+1] Gram diagonal sums
     unsigned int *d_queue = nullptr;           // [3 n_rep] task counters of gram_kernel
     // FFT estimator (ising3d_measure_radial): created on first use, library-owned
@@ -218,6 +220,23 @@ int sweep_generic(ising3d *h, uint64_t n)
                                                                      h->L, t, 0, mixed);
         ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
                                                                      h->L, t, 1, mixed);
+    }
+    h->launches += 2 * n;
+    CUDA_TRY(cudaGetLastError());
+    return ISING3D_OK;
+}
+
+int sweep_glauber(ising3d *h, uint64_t n)
+{
+    const size_t groups = h->words_per_replica() / 8;   // per colour
+    dim3 grid((unsigned)((groups + 255) / 256), (unsigned)h->n_rep);
+    const int mixed = h->cycle == ISING3D_CYCLE_MIXED;
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint32_t t = (uint32_t)(h->sweep + i);
+        ising::halfsweep_glauber_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds, h->L,
+                                                                     t, 0, mixed, h->glauber);
+        ising::halfsweep_glauber_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds, h->L,
+                                                                     t, 1, mixed, h->glauber);
     }
     h->launches += 2 * n;
     CUDA_TRY(cudaGetLastError());
@@ -431,11 +450,32 @@ int ising3d_set_measure_variant(ising3d_t *h, int variant)
     return ISING3D_OK;
 }
 
+int ising3d_set_temperature(ising3d_t *h, double T)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (!(T >= 0.0) || !std::isfinite(T)) return fail(ISING3D_EINVAL, "temperature must be finite and >= 0");
+    if (T > 0.0 && h->cycle == ISING3D_CYCLE_MIXED)
+        return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
+    h->temperature = T;
+    if (T > 0.0) {
+        // D13: thr[n] = floor(2^32 / (1 + exp((12 - 4n)/T))), fp64, n = antiparallel neighbours
+        for (int n = 0; n <= 6; ++n) {
+            const double dE = 12.0 - 4.0 * (double)n;
+            const double p = 1.0 / (1.0 + std::exp(dE / T));
+            const uint64_t thr = (uint64_t)std::floor(p * 4294967296.0);
+            for (int B = 0; B <= 32; ++B) h->glauber.sel[B][n] = ((thr >> B) & 1u) ? 0xFFFFFFFFu : 0u;
+        }
+    }
+    return ISING3D_OK;
+}
+
 int ising3d_set_cycle(ising3d_t *h, int cycle)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     if (cycle != ISING3D_CYCLE_01 && cycle != ISING3D_CYCLE_MIXED)
         return fail(ISING3D_EINVAL, "unknown cycle");
+    if (cycle == ISING3D_CYCLE_MIXED && h->temperature > 0.0)
+        return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     if (cycle == ISING3D_CYCLE_MIXED && h->variant == ISING3D_VARIANT_FUSED)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
     h->cycle = cycle;
@@ -481,7 +521,8 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xFFFFFFFFull || h->sweep + n_sweeps < h->sweep)
         return fail(ISING3D_EINVAL, "sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return ISING3D_OK;
-    const int rc = h->use_resident() ? sweep_resident(h, n_sweeps)
+    const int rc = h->temperature > 0.0 ? sweep_glauber(h, n_sweeps)
+                   : h->use_resident() ? sweep_resident(h, n_sweeps)
                    : h->use_fused2()  ? sweep_fused(h, n_sweeps, true)
                    : h->use_fused() ? sweep_fused(h, n_sweeps, false)
                                     : sweep_generic(h, n_sweeps);
@@ -678,6 +719,7 @@ const char *ising3d_measure_variant_name(const ising3d_t *h)
 const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";
+    if (h->temperature > 0.0) return "glauber";
     return h->use_resident() ? "resident" : h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
 }
 

@@ -122,4 +122,94 @@ halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
     reinterpret_cast<uint4 *>(own)[g] = make_uint4(out[0], out[1], out[2], out[3]);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Finite-temperature Glauber half-sweep (eq. (5); reading D13).
+// A site with n antiparallel neighbours flips iff u < thr[n], u its 32-bit uniform of the sweep,
+// thr[n] = floor(2^32 / (1 + exp((12 - 4n)/T))) in [0, 2^32].  Bit-sliced: n is counted with two
+// 3:2 compressors (c2 c1 c0), the seven class masks are one LOP3 each, and u < thr[n] is decided
+// MSB first over bit planes: plane j of u for the 128 spins of a group is one Philox call
+// (counter (q, t, colour, 4 + j)), the threshold's bit of that plane is a 7-entry truth table over
+// n (GlauberTables, built on the host).  The loop stops as soon as no site of the warp is still
+// undecided (about 13 of 32 planes on average), which is exact: later planes cannot change lt.
+// ---------------------------------------------------------------------------------------------
+struct GlauberTables {
+    uint32_t sel[33][7];     // sel[B][n] = all ones iff bit B (32 = the 2^32 bit, .. 0) of thr[n] is set
+};
+
+__global__ void __launch_bounds__(256)
+halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds, int L,
+                         uint32_t t, int phase, int mixed, const __grid_constant__ GlauberTables tb)
+{
+    const int WPR = L >> 6;
+    const size_t WPC = (size_t)L * L * WPR;
+    const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = g < WPC / 4;
+    const size_t gg = active ? g : 0;                           // idle lanes follow along (warp votes)
+    const int rep = blockIdx.y;
+    const uint64_t seed = seeds[rep];
+    const int c = mixed ? phase ^ first_colour(seed, t) : phase;
+    uint32_t *own = state + (size_t)rep * 2 * WPC + (size_t)c * WPC;
+    const uint32_t *oth = state + (size_t)rep * 2 * WPC + (size_t)(1 - c) * WPC;
+    const uint4 sv = reinterpret_cast<const uint4 *>(own)[gg];
+    const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+    uint32_t cls[4][7];                                         // class masks: n == 0..6
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const size_t w = 4 * gg + i;
+        const int wi = (int)(w % WPR);
+        const size_t row = w / WPR;
+        const int y = (int)(row % L), z = (int)(row / L);
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const uint32_t n_same = oth[w];
+        uint32_t n_x;
+        if (((y + z + c) & 1) == 0) {
+            const uint32_t prev = oth[row * WPR + (wi == 0 ? WPR - 1 : wi - 1)];
+            n_x = (n_same << 1) | (prev >> 31);
+        } else {
+            const uint32_t next = oth[row * WPR + (wi == WPR - 1 ? 0 : wi + 1)];
+            n_x = (n_same >> 1) | (next << 31);
+        }
+        // antiparallel indicators of the six neighbours
+        const uint32_t d1 = s[i] ^ n_same, d2 = s[i] ^ n_x;
+        const uint32_t d3 = s[i] ^ oth[((size_t)z * L + yp) * WPR + wi];
+        const uint32_t d4 = s[i] ^ oth[((size_t)z * L + ym) * WPR + wi];
+        const uint32_t d5 = s[i] ^ oth[((size_t)zp * L + y) * WPR + wi];
+        const uint32_t d6 = s[i] ^ oth[((size_t)zm * L + y) * WPR + wi];
+        const uint32_t sa = d1 ^ d2 ^ d3, ca = maj3(d1, d2, d3);
+        const uint32_t sb = d4 ^ d5 ^ d6, cb = maj3(d4, d5, d6);
+        const uint32_t c0 = sa ^ sb, k1 = sa & sb;
+        const uint32_t c1 = ca ^ cb ^ k1, c2 = maj3(ca, cb, k1);
+#pragma unroll
+        for (int n = 0; n < 7; ++n)
+            cls[i][n] = ((n & 1) ? c0 : ~c0) & ((n & 2) ? c1 : ~c1) & ((n & 4) ? c2 : ~c2);
+    }
+    uint32_t lt[4], eq[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {                               // the 2^32 bit: u has none
+        uint32_t T = 0;
+#pragma unroll
+        for (int n = 0; n < 7; ++n) T |= cls[i][n] & tb.sel[32][n];
+        lt[i] = T;
+        eq[i] = ~T;
+    }
+    for (int j = 0; j < 32; ++j) {
+        const uint32_t alive = active ? (eq[0] | eq[1] | eq[2] | eq[3]) : 0u;
+        if (!__any_sync(0xffffffffu, alive != 0u)) break;
+        const uint4 rnd = philox4x32_10((uint32_t)gg, t, (uint32_t)c, 4u + (uint32_t)j, (uint32_t)seed,
+                                        (uint32_t)(seed >> 32));
+        const uint32_t r[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            uint32_t T = 0;
+#pragma unroll
+            for (int n = 0; n < 7; ++n) T |= cls[i][n] & tb.sel[31 - j][n];
+            lt[i] |= eq[i] & ~r[i] & T;
+            eq[i] &= ~(r[i] ^ T);
+        }
+    }
+    if (active)
+        reinterpret_cast<uint4 *>(own)[g] = make_uint4(s[0] ^ lt[0], s[1] ^ lt[1], s[2] ^ lt[2], s[3] ^ lt[3]);
+}
+
 }  // namespace ising

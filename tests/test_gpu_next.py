@@ -256,3 +256,66 @@ def test_radial_estimator_large_identities(B):
     assert abs(r["C_rad"][0][1] - m["C"][0][1]) < 0.1
     assert abs(r["ell"][0] - m["ell"][0]) < 0.25 * m["ell"][0]
     sim.free()
+
+
+# ------------------------------------------------------------------ f-4: finite-temperature Glauber
+@pytest.mark.parametrize("L,seed,T,cps", [(64, 1, 4.0, [1, 2, 5]), (64, 2, 1.5, [1, 4]), (64, 3, 0.3, [2]),
+                                          (128, 7, 4.51, [1, 3]), (192, 8, 2.0, [2]), (64, 9, 1e9, [1, 3])])
+def test_glauber_against_oracle(B, orc, L, seed, T, cps):
+    sim = B.Ising3D(L, [seed])
+    sim.set_temperature(T)
+    assert sim.variant_name == "glauber"
+    ref = orc.Oracle(L, seed)
+    t = 0
+    for cp in cps:
+        sim.sweep(cp - t)
+        ref.sweep_T(cp - t, T)
+        t = cp
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+    check_measure(sim.measure(), ref.measure_full())
+    # back to T = 0: the quench continues with the paper's rule
+    sim.set_temperature(0.0)
+    assert sim.variant_name != "glauber"
+    sim.sweep(2)
+    ref.sweep(2)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    sim.free()
+
+
+def test_glauber_batch_and_errors(B, orc):
+    L, seeds, T = 64, [100, 101, 163], 3.0
+    batch = B.Ising3D(L, seeds)
+    batch.set_temperature(T)
+    batch.sweep(3)
+    st = batch.get_state().reshape(3, -1)
+    for i, s in enumerate(seeds):
+        ref = orc.Oracle(L, s)
+        ref.sweep_T(3, T)
+        assert np.array_equal(st[i], ref.export_words())
+    with pytest.raises(B.Ising3DError):
+        batch.set_temperature(-1.0)
+    with pytest.raises(B.Ising3DError):
+        batch.set_temperature(float("nan"))
+    with pytest.raises(B.Ising3DError):
+        batch.set_cycle(B.CYCLE_MIXED)            # T > 0 runs the 01 cycle only
+    batch.free()
+
+
+def test_glauber_full_size_properties(B):
+    """L = 1024 at T = 2: properties that hold at any size -- first half-sweep from the all-up
+    state flips a fraction p(0) of colour 0 and leaves colour 1 alone (closed form, binomial)."""
+    import math
+    L, T = 1024, 2.0
+    sim = B.Ising3D(L, [5], variant=B.VARIANT_GENERIC)
+    sim.set_temperature(T)
+    words = np.full(L ** 3 // 32, 0xFFFFFFFF, dtype=np.uint32)
+    sim.set_state(words, 0)
+    sim.sweep(1)
+    m = sim.measure()
+    N = L ** 3
+    p0 = 1.0 / (1.0 + math.exp(12.0 / T))
+    # after one full sweep from all-up nearly all flips are isolated (p0 = 2.5e-3): the number of
+    # down spins is N p0 up to corrections of relative order 6 p0 and binomial noise
+    n_down = N - int(m["n_up"][0])
+    assert abs(n_down - N * p0) < 0.05 * N * p0
+    sim.free()
