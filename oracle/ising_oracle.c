@@ -41,6 +41,9 @@
  *                         P along the axes = N - 2 A_mu(r) (orc_measure), slab closed form,
  *                         shell counts against a set-based Python count, bins vs exact
  *                         rational comparison
+ *   orc_half_sweep_dcb / orc_sweep_dcb : B = L reduces to the plain 01 sweep, pure-Python
+ *                         restatement on L = 8, every site proposed once (Neel read-out per
+ *                         block colour), fixed points, energy monotone
  *   orc_glauber_thresholds / orc_site_uniform / orc_sweep_T : p(6-n) = 1 - p(n), p(3) = 1/2,
  *                         hand-computed thresholds, T -> infinity closed form (flip iff the top
  *                         Philox plane bit is 0), acceptance frequencies on uniform-n states
@@ -272,6 +275,42 @@ void orc_sweep_mixed(orc_t *o, uint64_t n_sweeps)
         int first = orc_first_colour(o->seed, o->sweep);
         orc_half_sweep(o, o->sweep, first, 0, 0);
         orc_half_sweep(o, o->sweep, 1 - first, 0, 0);
+        o->sweep += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* Double-checkerboard update, 01 cycle (Supp. I.A    */
+/* PAPER.md:223-240): the lattice is cut into cubic blocks forming a    */
+/* coarse checkerboard; one sweep = kernel on the red blocks (update    */
+/* the darker sites of each block, barrier, the lighter sites, write    */
+/* back), then the same on the blue blocks.  While a coarse colour is   */
+/* being updated its halo in the other blocks is frozen, so the sweep   */
+/* is four masked half-sweeps: (coarse 0, fine 0), (coarse 0, fine 1),  */
+/* (coarse 1, fine 0), (coarse 1, fine 1).  Reading D14: block edge B   */
+/* (the paper gives none; the library uses B = 8), blocks start at the  */
+/* origin, coarse colour = (x/B + y/B + z/B) mod 2 (L/B even), fine     */
+/* colour = (x+y+z) mod 2 ("darker" = 0), red = coarse 0 first; tie bit */
+/* of a site = its Philox bit with counter (q, t, fine colour, 0) as in */
+/* the plain checkerboard: every site is proposed once per sweep.       */
+/* ------------------------------------------------------------------ */
+void orc_half_sweep_dcb(orc_t *o, uint32_t t, int coarse, int fine, int B)
+{
+    const int L = o->L;
+    #pragma omp parallel for schedule(static)
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x)
+                if (((x + y + z) & 1) == fine && ((x / B + y / B + z / B) & 1) == coarse)
+                    orc_update_site(o, x, y, z, t);
+}
+
+void orc_sweep_dcb(orc_t *o, uint64_t n_sweeps, int B)
+{
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        for (int coarse = 0; coarse < 2; ++coarse)
+            for (int fine = 0; fine < 2; ++fine)
+                orc_half_sweep_dcb(o, o->sweep, coarse, fine, B);
         o->sweep += 1;
     }
 }

@@ -103,6 +103,10 @@ def lib():
         l.orc_corr_direct.restype = None
         l.orc_radial_sums.argtypes = [C.c_int, i64p, i64p, u64p]
         l.orc_radial_sums.restype = None
+        l.orc_half_sweep_dcb.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_int, C.c_int]
+        l.orc_half_sweep_dcb.restype = None
+        l.orc_sweep_dcb.argtypes = [C.c_void_p, C.c_uint64, C.c_int]
+        l.orc_sweep_dcb.restype = None
         l.orc_glauber_thresholds.argtypes = [C.c_double, u64p]
         l.orc_glauber_thresholds.restype = None
         l.orc_site_uniform.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint32]
@@ -313,6 +317,14 @@ class Oracle:
                 ell = r + (C_rad[r] - c_intercept) / (C_rad[r] - C_rad[r + 1])
                 break
         return {"corr_sum": sums, "shell": cnt, "C_rad": C_rad, "S_rad": S_rad, "ell": ell, "m": m}
+
+    def sweep_dcb(self, n: int = 1, block: int = 8):
+        """n sweeps of the double-checkerboard 01 cycle (Supp. I.A, D14), block edge `block`."""
+        assert self.L % (2 * block) == 0 or block >= self.L
+        self._l.orc_sweep_dcb(self._h, int(n), int(block))
+
+    def half_sweep_dcb(self, t: int, coarse: int, fine: int, block: int = 8):
+        self._l.orc_half_sweep_dcb(self._h, int(t), int(coarse), int(fine), int(block))
 
     def sweep_T(self, n: int, T: float):
         """n sweeps of finite-temperature Glauber dynamics (eq. (5), D13)."""

@@ -369,3 +369,69 @@ def test_glauber_cold_limit_and_relaxation():
     assert np.array_equal(c.spins, d.spins) and c.sweep_count == 12
     e1 = c.measure([1])[1].sum()
     assert 0 < e1 < 0.45 * e0
+
+
+# ------------------------------------------------------------------ f-2: double checkerboard
+def test_double_checkerboard_reduces_to_plain_sweep():
+    """One block (B >= L): the coarse colour is 0 everywhere, the sweep is (fine 0, fine 1) and
+    nothing else: the plain 01 sweep."""
+    L = 12
+    a = orc.Oracle(L, 6)
+    b = orc.Oracle(L, 6)
+    a.sweep_dcb(5, block=L)
+    b.sweep(5)
+    assert np.array_equal(a.spins, b.spins) and a.sweep_count == 5
+
+
+def test_double_checkerboard_python_restatement():
+    """Pure-Python statement of Supp. I.A on L = 8, B = 4: red blocks (dark, then light), then
+    blue blocks, sites visited one by one with the Delta-E rule and the site's Philox bit."""
+    from test_oracle_pins import py_site_bit
+    L, B, seed = 8, 4, 31
+    o = orc.Oracle(L, seed)
+    s = o.spins.copy().astype(int)                       # [z][y][x]
+    for t in range(3):
+        for coarse in (0, 1):
+            for fine in (0, 1):
+                for z in range(L):
+                    for y in range(L):
+                        for x in range(L):
+                            if (x + y + z) % 2 != fine or (x // B + y // B + z // B) % 2 != coarse:
+                                continue
+                            h = (s[z][y][(x + 1) % L] + s[z][y][(x - 1) % L] + s[z][(y + 1) % L][x]
+                                 + s[z][(y - 1) % L][x] + s[(z + 1) % L][y][x] + s[(z - 1) % L][y][x])
+                            dE = 2 * s[z][y][x] * h
+                            if dE < 0 or (dE == 0 and py_site_bit(seed, L, x, y, z, t, 0)):
+                                s[z][y][x] = -s[z][y][x]
+    o.sweep_dcb(3, block=B)
+    assert np.array_equal(o.spins, s.astype(np.int8))
+
+
+def test_double_checkerboard_order_readout_and_invariants():
+    """From the Neel state the first phase (red blocks, dark sites) flips exactly the dark sites
+    of the red blocks (n = 6) and nothing else; the dark sites of the blue blocks bordering a red
+    block have then lost antiparallel neighbours.  Every phase only lowers the energy; all-up and
+    slab states are fixed points."""
+    L, B = 16, 4
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    fine = (x + y + z) & 1
+    coarse = (x // B + y // B + z // B) & 1
+    o = orc.Oracle(L, 2, init=False)
+    o.spins[...] = inputs.neel(L)
+    o.half_sweep_dcb(0, 0, 0, B)
+    want = inputs.neel(L).copy()
+    want[(fine == 0) & (coarse == 0)] *= -1
+    assert np.array_equal(o.spins, want)
+    o = orc.Oracle(L, 3)
+    e = o.measure([1])[1].sum()
+    for t in range(4):
+        for c in (0, 1):
+            for f in (0, 1):
+                o.half_sweep_dcb(t, c, f, B)
+                e2 = o.measure([1])[1].sum()
+                assert e2 <= e
+                e = e2
+    for s0 in (inputs.all_up(L), inputs.slab(L, 1, 2, L // 2)):
+        o.spins[...] = s0
+        o.sweep_dcb(3, block=B)
+        assert np.array_equal(o.spins, s0)
