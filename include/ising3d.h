@@ -87,6 +87,7 @@ extern "C" {
 /* update order inside a sweep (ising3d_set_cycle) */
 #define ISING3D_CYCLE_01    0   /* colour 0 then colour 1, every sweep (main text) */
 #define ISING3D_CYCLE_MIXED 1   /* first colour drawn per sweep (Supp. I.B PAPER.md:258, D10)    */
+#define ISING3D_CYCLE_DOUBLE_CB 2 /* double checkerboard, 01 cycle (Supp. I.A PAPER.md:223-240, D14) */
 
 typedef struct ising3d ising3d_t;   /* opaque */
 
@@ -166,8 +167,14 @@ int ising3d_init_menger(ising3d_t *h, int k);
  * which sublattice to update first ... still every spin is proposed to flip exactly once per
  * sweep"; reading D10): in sweep t the replica with seed s updates first the colour given by
  * bit 0 of word 0 of Philox(key = s, counter = (0, t, 0, 2)); the tie bits keep counter
- * (q, t, c, 0) with c the colour being updated.  Takes effect from the next sweep.
- * EINVAL for an unknown value or with ISING3D_VARIANT_FUSED (01 cycle only).
+ * (q, t, c, 0) with c the colour being updated.  Double checkerboard (Supp. I.A PAPER.md:223-240;
+ * reading D14): cubic blocks of edge 8 starting at the origin form a coarse checkerboard
+ * (coarse colour (x/8 + y/8 + z/8) mod 2); a sweep updates the red blocks (their darker sites,
+ * (x+y+z) even, then their lighter sites) with everything else frozen, then the blue blocks:
+ * four masked half-sweeps, every spin proposed once, tie bits as in the plain checkerboard.
+ * Runs on the resident (L <= 256) and generic kernels.  Takes effect from the next sweep.
+ * EINVAL for an unknown value, with ISING3D_VARIANT_FUSED (01 cycle only), for the double
+ * checkerboard with ISING3D_VARIANT_FUSED2, or at T > 0 for anything but the 01 cycle.
  */
 int ising3d_set_cycle(ising3d_t *h, int cycle);
 

@@ -108,13 +108,14 @@ struct ising3d {
     }
     bool use_fused2() const
     {
+        if (cycle == ISING3D_CYCLE_DOUBLE_CB) return false;     // four masked phases: resident / generic
         return variant == ISING3D_VARIANT_FUSED2 || (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
     bool use_fused() const
     {
+        if (cycle != ISING3D_CYCLE_01) return false;
         return variant == ISING3D_VARIANT_FUSED ||
-               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok() && !resident_ok() &&
-                cycle == ISING3D_CYCLE_01);
+               (variant == ISING3D_VARIANT_AUTO && fused_ok() && !fused2_ok() && !resident_ok());
     }
 };
 
@@ -216,10 +217,19 @@ int sweep_generic(ising3d *h, uint64_t n)
     const int mixed = h->cycle == ISING3D_CYCLE_MIXED;
     for (uint64_t i = 0; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
+        if (h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
+            // red blocks: dark sites, light sites; then the blue blocks (Supp. I.A, D14)
+            for (int coarse = 0; coarse < 2; ++coarse)
+                for (int fine = 0; fine < 2; ++fine)
+                    ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(
+                        h->state[h->cur], h->d_seeds, h->L, t, fine, 0, coarse);
+            h->launches += 2;
+            continue;
+        }
         ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
-                                                                     h->L, t, 0, mixed);
+                                                                     h->L, t, 0, mixed, -1);
         ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(h->state[h->cur], h->d_seeds,
-                                                                     h->L, t, 1, mixed);
+                                                                     h->L, t, 1, mixed, -1);
     }
     h->launches += 2 * n;
     CUDA_TRY(cudaGetLastError());
@@ -246,8 +256,7 @@ int sweep_glauber(ising3d *h, uint64_t n)
 int sweep_resident(ising3d *h, uint64_t n)
 {
     cudaError_t e = ising::launch_resident(h->state[h->cur], h->d_seeds, h->L, h->n_rep, h->res_plan,
-                                           (uint32_t)h->sweep, (uint32_t)n,
-                                           h->cycle == ISING3D_CYCLE_MIXED, h->stream);
+                                           (uint32_t)h->sweep, (uint32_t)n, h->cycle, h->stream);
     if (e != cudaSuccess)
         return fail(ISING3D_ECUDA, std::string("resident sweep launch: ") + cudaGetErrorString(e));
     h->launches += 1;
@@ -454,7 +463,7 @@ int ising3d_set_temperature(ising3d_t *h, double T)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     if (!(T >= 0.0) || !std::isfinite(T)) return fail(ISING3D_EINVAL, "temperature must be finite and >= 0");
-    if (T > 0.0 && h->cycle == ISING3D_CYCLE_MIXED)
+    if (T > 0.0 && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     h->temperature = T;
     if (T > 0.0) {
@@ -472,12 +481,14 @@ int ising3d_set_temperature(ising3d_t *h, double T)
 int ising3d_set_cycle(ising3d_t *h, int cycle)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (cycle != ISING3D_CYCLE_01 && cycle != ISING3D_CYCLE_MIXED)
+    if (cycle != ISING3D_CYCLE_01 && cycle != ISING3D_CYCLE_MIXED && cycle != ISING3D_CYCLE_DOUBLE_CB)
         return fail(ISING3D_EINVAL, "unknown cycle");
-    if (cycle == ISING3D_CYCLE_MIXED && h->temperature > 0.0)
+    if (cycle != ISING3D_CYCLE_01 && h->temperature > 0.0)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
-    if (cycle == ISING3D_CYCLE_MIXED && h->variant == ISING3D_VARIANT_FUSED)
+    if (cycle != ISING3D_CYCLE_01 && h->variant == ISING3D_VARIANT_FUSED)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
+    if (cycle == ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED2)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     h->cycle = cycle;
     return ISING3D_OK;
 }
@@ -503,7 +514,9 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_RESIDENT)
         return fail(ISING3D_EINVAL, "unknown variant");
-    if (variant == ISING3D_VARIANT_FUSED && h->cycle == ISING3D_CYCLE_MIXED)
+    if (variant == ISING3D_VARIANT_FUSED2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+    if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
         return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");

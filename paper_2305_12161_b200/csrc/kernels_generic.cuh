@@ -25,6 +25,7 @@ init_spins_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ see
     reinterpret_cast<uint4 *>(state)[(size_t)rep * 2 * groups_per_colour + g] = v;
 }
 
+// `coarse` >= 0: only the sites of that coarse colour are updated (double checkerboard, D14).
 // `phase` = 0 / 1: first / second half-sweep of sweep t.  01 cycle (mixed = 0): colour = phase.
 // Mixed cycle (mixed = 1, D10): colour = phase ^ first_colour(seed of the replica, t).
 // Menger-sponge start (D11): the lattice is tiled from the origin by sponges of
@@ -78,7 +79,7 @@ init_menger_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ se
 
 __global__ void __launch_bounds__(256)
 halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
-                         int L, uint32_t t, int phase, int mixed)
+                         int L, uint32_t t, int phase, int mixed, int coarse)
 {
     const int WPR = L >> 6;                                   // words per row
     const size_t WPC = (size_t)L * L * WPR;                   // words per colour
@@ -117,7 +118,9 @@ halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
             const uint32_t next = oth[row * WPR + (wi == WPR - 1 ? 0 : wi + 1)];
             n_x = (n_same >> 1) | (next << 31);
         }
-        out[i] = rule_word(s[i], rho[i], n_same, n_x, n_yp, n_ym, n_zp, n_zm);
+        const uint32_t upd = rule_word(s[i], rho[i], n_same, n_x, n_yp, n_ym, n_zp, n_zm);
+        const uint32_t m = dcb_mask(y, z, coarse);              // double checkerboard: one coarse colour
+        out[i] = (upd & m) | (s[i] & ~m);
     }
     reinterpret_cast<uint4 *>(own)[g] = make_uint4(out[0], out[1], out[2], out[3]);
 }

@@ -37,7 +37,8 @@ constexpr int kResThreads = 512;
 template <int WPR>
 __device__ __forceinline__ uint4 res_update_group(const uint4 own, const uint4 prv, const uint4 sam,
                                                   const uint4 nxt, const uint4 zm, const uint4 zp,
-                                                  const uint4 rho, const int par)
+                                                  const uint4 rho, const int par, const int y0,
+                                                  const int z, const int coarse)
 {
     // cmb[4 + i] = word i of the same group position, other colour, plane z; cmb[0..3] the
     // previous group of the plane, cmb[8..11] the next one (periodic in y)
@@ -60,7 +61,9 @@ __device__ __forceinline__ uint4 res_update_group(const uint4 own, const uint4 p
         const int o = (par + i / WPR) & 1;
         const uint32_t n_x = o ? __funnelshift_r(n_same, w_next, 1)     // neighbour k+1
                                : __funnelshift_l(w_prev, n_same, 1);    // neighbour k-1
-        out[i] = rule_word(s[i], r4[i], n_same, n_x, n_yp, n_ym, p[i], m[i]);
+        const uint32_t upd = rule_word(s[i], r4[i], n_same, n_x, n_yp, n_ym, p[i], m[i]);
+        const uint32_t msk = dcb_mask(y0 + i / WPR, z, coarse);   // double checkerboard phases (D14)
+        out[i] = (upd & msk) | (s[i] & ~msk);
     }
     return make_uint4(out[0], out[1], out[2], out[3]);
 }
@@ -69,7 +72,7 @@ __device__ __forceinline__ uint4 res_update_group(const uint4 own, const uint4 p
 template <int WPR>
 __global__ void __launch_bounds__(kResThreads, 1)
 resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
-                      const uint32_t t0, const uint32_t n_sweeps, const int mixed)
+                      const uint32_t t0, const uint32_t n_sweeps, const int cycle)
 {
     constexpr int L = 64 * WPR;
     constexpr int GPP = L * WPR / 4;              // 128-bit groups per plane
@@ -129,7 +132,7 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
 
     // one half-sweep of compile-time colour C (the compiler then folds the colour into the
     // smem offsets and the Philox counter)
-    auto half_sweep = [&](auto colour, const uint32_t t) {
+    auto half_sweep = [&](auto colour, const uint32_t t, const int coarse) {
         constexpr int C = decltype(colour)::value;
         uint4 *own = res_smem + (size_t)C * CSTRIDE;
         const uint4 *oth = res_smem + (size_t)(1 - C) * CSTRIDE;
@@ -142,7 +145,7 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
                 const uint4 o4 = own[(size_t)(zl + 1) * GPP + g];
                 const uint32_t q = (uint32_t)z * GPP + g;
                 const uint4 rho = philox4x32_10(q, t, (uint32_t)C, kTagTie, keys);
-                const uint4 nw = res_update_group<WPR>(o4, prv, sam, nxt, zm, zp, rho, (y0 + z + C) & 1);
+                const uint4 nw = res_update_group<WPR>(o4, prv, sam, nxt, zm, zp, rho, (y0 + z + C) & 1, y0, z, coarse);
                 own[(size_t)(zl + 1) * GPP + g] = nw;
                 if (zl == 0) peer_dn[(size_t)C * CSTRIDE + (size_t)(PZ + 1) * GPP + g] = nw;
                 if (zl == PZ - 1) peer_up[(size_t)C * CSTRIDE + g] = nw;
@@ -156,12 +159,17 @@ resident_sweep_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__
     for (uint32_t it = 0; it < n_sweeps; ++it) {
         const uint32_t t = t0 + it;
         // 01 cycle: colour 0 first (D7); mixed cycle: the first colour is drawn per sweep (D10)
-        if (mixed && first_colour(seed, t)) {
-            half_sweep(Colour1{}, t);
-            half_sweep(Colour0{}, t);
+        if (cycle == 2) {                 // double checkerboard: red blocks (dark, light), then blue
+            half_sweep(Colour0{}, t, 0);
+            half_sweep(Colour1{}, t, 0);
+            half_sweep(Colour0{}, t, 1);
+            half_sweep(Colour1{}, t, 1);
+        } else if (cycle == 1 && first_colour(seed, t)) {
+            half_sweep(Colour1{}, t, -1);
+            half_sweep(Colour0{}, t, -1);
         } else {
-            half_sweep(Colour0{}, t);
-            half_sweep(Colour1{}, t);
+            half_sweep(Colour0{}, t, -1);
+            half_sweep(Colour1{}, t, -1);
         }
     }
 
@@ -244,7 +252,7 @@ inline ResidentPlan resident_plan(int L, int n_rep, int sm_count)
 template <int WPR>
 inline cudaError_t launch_resident_t(uint32_t *state, const uint64_t *d_seeds, int n_rep,
                                      const ResidentPlan &plan, uint32_t t0, uint32_t n_sweeps,
-                                     int mixed, cudaStream_t stream)
+                                     int cycle, cudaStream_t stream)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)plan.cs, (unsigned)n_rep);
@@ -258,17 +266,17 @@ inline cudaError_t launch_resident_t(uint32_t *state, const uint64_t *d_seeds, i
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, resident_sweep_kernel<WPR>, state, d_seeds, t0, n_sweeps, mixed);
+    return cudaLaunchKernelEx(&cfg, resident_sweep_kernel<WPR>, state, d_seeds, t0, n_sweeps, cycle);
 }
 
 inline cudaError_t launch_resident(uint32_t *state, const uint64_t *d_seeds, int L, int n_rep,
                                    const ResidentPlan &plan, uint32_t t0, uint32_t n_sweeps,
-                                   int mixed, cudaStream_t stream)
+                                   int cycle, cudaStream_t stream)
 {
     switch (L) {
-        case 64:  return launch_resident_t<1>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
-        case 128: return launch_resident_t<2>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
-        case 256: return launch_resident_t<4>(state, d_seeds, n_rep, plan, t0, n_sweeps, mixed, stream);
+        case 64:  return launch_resident_t<1>(state, d_seeds, n_rep, plan, t0, n_sweeps, cycle, stream);
+        case 128: return launch_resident_t<2>(state, d_seeds, n_rep, plan, t0, n_sweeps, cycle, stream);
+        case 256: return launch_resident_t<4>(state, d_seeds, n_rep, plan, t0, n_sweeps, cycle, stream);
         default:  return cudaErrorInvalidValue;
     }
 }

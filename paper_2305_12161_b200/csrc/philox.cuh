@@ -87,6 +87,18 @@ __host__ __device__ __forceinline__ int first_colour(uint64_t seed, uint32_t t)
     return (int)(philox4x32_10(0u, t, 0u, kTagOrder, (uint32_t)seed, (uint32_t)(seed >> 32)).x & 1u);
 }
 
+// Double checkerboard (Supp. I.A PAPER.md:223-240, D14): cubic blocks of edge kDcbBlock form a
+// coarse checkerboard; a phase updates the sites of one coarse colour only.  For the word
+// (y, z) of either fine colour, bit j is site k = 32 wi + j, x = 2k + o, so x / 8 = 8 wi + j / 4:
+// the sites of coarse colour `coarse` are the bits with ((j >> 2) + (y >> 3) + (z >> 3)) & 1 ==
+// coarse.  coarse < 0: no mask (plain checkerboard).
+constexpr int kDcbBlock = 8;
+__device__ __forceinline__ uint32_t dcb_mask(int y, int z, int coarse)
+{
+    if (coarse < 0) return 0xFFFFFFFFu;
+    return (((y >> 3) + (z >> 3) + coarse) & 1) ? 0xF0F0F0F0u : 0x0F0F0F0Fu;
+}
+
 // ---------------------------------------------------------------------------
 // The site rule on 32 sites at once (eq. (6), D2).
 // n1..n6: the six neighbour words (bit = 1 <=> spin up), s: own word, rho: tie bits.

@@ -319,3 +319,47 @@ def test_glauber_full_size_properties(B):
     n_down = N - int(m["n_up"][0])
     assert abs(n_down - N * p0) < 0.05 * N * p0
     sim.free()
+
+
+# ------------------------------------------------------------------ f-2: double checkerboard
+@pytest.mark.parametrize("L,seed,variant,cps", [(64, 1, "auto", [1, 2, 6]), (128, 7, "auto", [1, 5]),
+                                                (256, 2, "auto", [2, 4]), (192, 8, "auto", [1, 3]),
+                                                (64, 3, "generic", [1, 4]), (512, 11, "auto", [1, 2])])
+def test_double_checkerboard_against_oracle(B, orc, L, seed, variant, cps):
+    sim = B.Ising3D(L, [seed], variant=VARIANTS(B)[variant])
+    sim.set_cycle(B.CYCLE_DOUBLE_CB)
+    assert sim.variant_name in ("resident", "generic")
+    ref = orc.Oracle(L, seed)
+    t = 0
+    for cp in cps:
+        sim.sweep(cp - t)
+        ref.sweep_dcb(cp - t, block=8)
+        t = cp
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+    if L <= 256:
+        check_measure(sim.measure(), ref.measure_full())
+    sim.set_cycle(B.CYCLE_01)                      # and back to the main-text cycle
+    sim.sweep(1)
+    ref.sweep(1)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    sim.free()
+
+
+def test_double_checkerboard_batch_neel_and_errors(B, orc):
+    L = 128
+    batch = B.Ising3D(L, [100, 163])
+    batch.set_cycle(B.CYCLE_DOUBLE_CB)
+    batch.sweep(3)
+    st = batch.get_state().reshape(2, -1)
+    for i, s in enumerate((100, 163)):
+        ref = orc.Oracle(L, s)
+        ref.sweep_dcb(3, block=8)
+        assert np.array_equal(st[i], ref.export_words())
+    batch.free()
+    sim = B.Ising3D(512, [1])
+    sim.set_cycle(B.CYCLE_DOUBLE_CB)
+    with pytest.raises(B.Ising3DError):
+        sim.set_variant(B.VARIANT_FUSED2)
+    with pytest.raises(B.Ising3DError):
+        sim.set_temperature(2.0)
+    sim.free()
