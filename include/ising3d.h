@@ -72,7 +72,7 @@ extern "C" {
 #define ISING3D_ECUDA  (-3)   /* CUDA runtime error; text in ising3d_last_error()         */
 
 /* sweep-kernel variants (ising3d_set_variant) */
-#define ISING3D_VARIANT_AUTO    0   /* fused kernel where the shape allows, else generic */
+#define ISING3D_VARIANT_AUTO    0   /* resident (L <= 256), fused2 (L in 512..4096), else generic */
 #define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
 #define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
 #define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096)        */
@@ -208,7 +208,9 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);
 /*
  * Integer measurements + fp64 post-processing (D8, D9; eq. (2) PAPER.md:43,
  * ell from C = c PAPER.md:51).  Synchronises the handle's stream.  Does not
- * change the state or the sweep counter.
+ * change the state or the sweep counter.  The tensor-core variant uses the
+ * handle's second (ping-pong) state buffer as scratch; that buffer never holds
+ * live data between calls.
  */
 int ising3d_measure(ising3d_t *h, ising3d_meas_t *out);
 

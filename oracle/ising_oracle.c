@@ -634,6 +634,9 @@ void orc_export(const orc_t *o, uint32_t *words)
     const int L = o->L;
     size_t wpc = orc_words_per_colour(L);
     memset(words, 0, 2 * wpc * sizeof(uint32_t));
+    /* rows of L/2 bits start on word boundaries when L % 64 == 0: planes then touch disjoint
+     * words and may go in parallel (no arithmetic here, only the D3 format) */
+    #pragma omp parallel for schedule(static) if (L % 64 == 0)
     for (int z = 0; z < L; ++z)
         for (int y = 0; y < L; ++y)
             for (int x = 0; x < L; ++x) {
@@ -648,6 +651,7 @@ void orc_import(orc_t *o, const uint32_t *words, uint32_t sweep)
 {
     const int L = o->L;
     size_t wpc = orc_words_per_colour(L);
+    #pragma omp parallel for schedule(static)
     for (int z = 0; z < L; ++z)
         for (int y = 0; y < L; ++y)
             for (int x = 0; x < L; ++x) {

@@ -418,3 +418,32 @@ def test_measure_variant_errors(B):
     with pytest.raises(B.Ising3DError):
         sim.set_measure_variant(9)
     sim.free()
+
+
+# ------------------------------------------------------------------ configs 4 and 5: windows at full size
+@pytest.mark.parametrize("name,t_enter,n_window", [("config4_L1024", 1000, 4), ("config5_L2048", 1000, 2)])
+def test_full_size_window_against_oracle(B, orc, name, t_enter, n_window):
+    """the oracle cannot follow 10^5 sweeps of L = 1024 or anything long at
+    L = 2048, but the RNG is counter based, so a window entered through get_state is exact:
+    run the CUDA path to t_enter, hand the WHOLE state to the oracle, advance both by n_window
+    sweeps and compare every word, plus the counts on a thinned r set."""
+    w = inputs.WORKLOADS[name]
+    L, seed = w["L"], w["seeds"][0]
+    sim = B.Ising3D(L, [seed])
+    assert sim.variant_name == "fused2"
+    sim.sweep(t_enter)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    sim.get_state(buf)
+    ref = orc.Oracle(L, seed, init=False)
+    ref.import_words(buf, t_enter)
+    sim.sweep(n_window)
+    ref.sweep(n_window)
+    assert sim.sweep_count == ref.sweep_count == t_enter + n_window
+    assert np.array_equal(sim.get_state(buf), ref.export_words()), "window state differs"
+    thin = np.array([0, 1, 2, 3, 5, 8, 16, 33, 64, 128, 257, L // 4, L // 2 - 1, L // 2] if L <= 1024
+                    else [0, 1, 2, 3, 16, 257, L // 2 - 1, L // 2], dtype=np.int32)
+    got = sim.measure()
+    n_up, a = ref.measure(thin)
+    assert int(got["n_up"][0]) == n_up
+    assert np.array_equal(got["antipar"][0][:, thin], a)
+    sim.free()
