@@ -329,6 +329,9 @@ def run_ours(args):
         "hbm_bound_site_updates_per_ns": hbm_bound,
         "alu_bound_site_updates_per_ns": alu_bound,
         "frac_of_min_roofline": (N * S / (sweep_ms * 1e6)) / min(hbm_bound, alu_bound),
+        # the stricter view: the N/4 bytes per sweep a fused black+white pass cannot avoid moving
+        "frac_on_fused_floor_bytes": (0.25 * N / launches_per_sweep / (avg_launch_ms * 1e-3) / 1e9) / peak
+        if launches_per_sweep == 1 else None,
         "note": "algorithmic bytes = 3N/8 per sweep (two half-sweeps each read both colours' "
                 "share and write one); the fused kernel moves ~N/4 + halo, so frac can pass 1",
     }

@@ -421,7 +421,8 @@ def test_measure_variant_errors(B):
 
 
 # ------------------------------------------------------------------ configs 4 and 5: windows at full size
-@pytest.mark.parametrize("name,t_enter,n_window", [("config4_L1024", 1000, 4), ("config5_L2048", 1000, 2)])
+@pytest.mark.parametrize("name,t_enter,n_window", [("config4_L1024", 1000, 4), ("config4_L1024", 99_996, 4),
+                                                   ("config5_L2048", 1000, 2)])
 def test_full_size_window_against_oracle(B, orc, name, t_enter, n_window):
     """the oracle cannot follow 10^5 sweeps of L = 1024 or anything long at
     L = 2048, but the RNG is counter based, so a window entered through get_state is exact:
@@ -446,4 +447,19 @@ def test_full_size_window_against_oracle(B, orc, name, t_enter, n_window):
     n_up, a = ref.measure(thin)
     assert int(got["n_up"][0]) == n_up
     assert np.array_equal(got["antipar"][0][:, thin], a)
+    sim.free()
+
+
+def test_config5_from_the_start_full_state(B, orc):
+    """Config 5 at full size from its own T = infinity start: the oracle draws all 8.6e9 spins
+    from its own Philox, both sides sweep twice, every word is compared (not a sample)."""
+    w = inputs.WORKLOADS["config5_L2048"]
+    L, seed = w["L"], w["seeds"][0]
+    sim = B.Ising3D(L, [seed])
+    ref = orc.Oracle(L, seed)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    assert np.array_equal(sim.get_state(buf), ref.export_words()), "T = infinity start differs"
+    sim.sweep(2)
+    ref.sweep(2)
+    assert np.array_equal(sim.get_state(buf), ref.export_words()), "state differs after 2 sweeps"
     sim.free()
