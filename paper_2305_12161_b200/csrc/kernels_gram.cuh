@@ -17,9 +17,11 @@
 //                            (a site keeps its bit under a y/z shift and alternates colour), a
 //                            32x32 warp bit-transpose for x.
 //   gram_kernel              persistent CTAs, dynamic task queue; task = (128 positions a) x
-//                            (up to 4 units of 128 positions b = a0 + 128 u ...) x (a slice of K).
-//                            8 expander warps fill a 2-stage ring (full/empty mbarriers, generic
-//                            -> async proxy fence), warp 8 issues the MMAs and commits, the
+//                            (up to 3 units of 128 positions b = a0 + 128 u ...) x (a slice of K).
+//                            8 expander warps fill a 4-stage ring (full/empty mbarriers): the B
+//                            tiles go to shared memory (generic -> async proxy fence), the A tile
+//                            to tensor memory (tcgen05.st, so the tensor core reads only B from
+//                            shared memory); warp 8 issues the MMAs (A from TMEM) and commits; the
 //                            expander warps read the accumulators back (tcgen05.ld) and add
 //                            G[a][b] to a shared-memory histogram over r = b - a.
 //   gram_finalize_kernel     A_mu(r) = 2 N_up - 2 Gsum_mu(r).
@@ -33,10 +35,11 @@
 namespace ising {
 
 constexpr int kGramExpWarps = 8;                       // expander / epilogue warps
-constexpr int kGramRowsPerThread = (128 * (1 + 4) + kGramExpWarps * 32 - 1) / (kGramExpWarps * 32);
+constexpr int kGramRowsPerThread = (128 * (1 + 3) + kGramExpWarps * 32 - 1) / (kGramExpWarps * 32);
 constexpr int kGramThreads = (kGramExpWarps + 1) * 32;   // + the MMA warp
-constexpr int kGramMaxStages = 3;
-constexpr int kGramMaxUnits = 4;                       // 4 x 128 accumulator columns = all of TMEM
+constexpr int kGramMaxStages = 4;
+constexpr int kGramMaxUnits = 3;                       // 3 x 128 accumulator columns; the rest of TMEM holds A
+constexpr uint32_t kGramTmemA = 128u * kGramMaxUnits;  // first TMEM column of the A stages (32 columns each)
 constexpr int kGramTile = 128 * 128;                   // bytes of one 128-row operand tile (K = 128)
 
 inline bool gram_supported(int L) { return L >= 512 && (L % 512) == 0; }
@@ -132,6 +135,17 @@ __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t d
         : "memory");
 }
 
+// the same with the A operand in tensor memory (lane = row, 4 K-bytes per 32-bit column)
+__device__ __forceinline__ void umma_i8_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc,
+                                           uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}\n"
+        ::"r"(tmem_d), "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
 __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
@@ -170,6 +184,29 @@ __device__ __forceinline__ void expand_row(uint8_t *tile, const int row, const u
         }
     }
 }
+// An A row goes to tensor memory instead: the warp stores its 32 rows (lane = row) as 32 columns,
+// column 8 i + j = the four K-bytes of bit j of the bytes of line word i (the order expand_row<true>
+// gives the B rows in shared memory).  Halves the shared-memory traffic of the kernel: the tensor
+// core then reads only B from shared memory.
+__device__ __forceinline__ void expand_row_tmem(const uint32_t taddr, const uint4 w)
+{
+    const uint32_t in[4] = {w.x, w.y, w.z, w.w};
+    uint32_t a[32];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t v = __byte_perm(in[i], 0u, 0x0123u);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[8 * i + j] = v & (0x01010101u << j);
+    }
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]), "r"(a[7]),
+          "r"(a[8]), "r"(a[9]), "r"(a[10]), "r"(a[11]), "r"(a[12]), "r"(a[13]), "r"(a[14]), "r"(a[15]),
+          "r"(a[16]), "r"(a[17]), "r"(a[18]), "r"(a[19]), "r"(a[20]), "r"(a[21]), "r"(a[22]), "r"(a[23]),
+          "r"(a[24]), "r"(a[25]), "r"(a[26]), "r"(a[27]), "r"(a[28]), "r"(a[29]), "r"(a[30]), "r"(a[31])
+        : "memory");
+}
 constexpr int kGramProductShift = 7;       // accumulators = G << 7
 
 struct GramPlan {
@@ -177,7 +214,7 @@ struct GramPlan {
     int units[8];            // units (of 128 columns) per group
     int ustart[8];           // first unit of each group
     int max_units;           // largest group: a stage is (1 + max_units) tiles
-    int n_stages;            // ring depth (2 or 3, what fits shared memory)
+    int n_stages;            // ring depth (4: B tiles in shared memory, A tiles in tensor memory)
     int n_slices;            // K slices
     int n_tasks;             // n_slices * (L/128) * n_groups
 };
@@ -194,7 +231,7 @@ inline GramPlan make_gram_plan(int L, int sm_count)
         u += p.units[g];
     }
     p.max_units = p.units[0];
-    p.n_stages = (1 + p.max_units) * kGramTile * 3 <= 196 * 1024 ? 3 : 2;
+    p.n_stages = kGramMaxStages;
     const int tiles = (L / 128) * p.n_groups;
     p.n_slices = (sm_count * 12 + tiles - 1) / tiles;
     p.n_tasks = p.n_slices * tiles;
@@ -203,7 +240,7 @@ inline GramPlan make_gram_plan(int L, int sm_count)
 
 inline size_t gram_smem_bytes(int L, const GramPlan &p)
 {
-    return (size_t)p.n_stages * (1 + p.max_units) * kGramTile + (size_t)(L / 2 + 1) * 4 + 1024 + 256;
+    return (size_t)p.n_stages * p.max_units * kGramTile + (size_t)(L / 2 + 1) * 4 + 1024 + 256;
 }
 
 // ---- the Gram kernel ---------------------------------------------------------------------------
@@ -215,10 +252,10 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
 {
     extern __shared__ __align__(1024) uint8_t gram_raw[];
     uint8_t *smem = gram_raw + ((1024u - (smem_u32(gram_raw) & 1023u)) & 1023u);
-    // stage s: A tile, then max_units B tiles
+    // stage s: max_units B tiles in shared memory + 32 TMEM columns of A
     uint8_t *tiles = smem;
     const int NS = plan.n_stages;
-    const size_t stage_bytes = (size_t)(1 + plan.max_units) * kGramTile;
+    const size_t stage_bytes = (size_t)plan.max_units * kGramTile;   // B tiles only; A lives in TMEM
     uint32_t *hist = reinterpret_cast<uint32_t *>(smem + (size_t)NS * stage_bytes);
     __shared__ uint64_t full_bar[kGramMaxStages], empty_bar[kGramMaxStages], acc_full, acc_empty;
     __shared__ uint32_t tmem_base_s;
@@ -288,7 +325,7 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
                 }
                 if (pos >= L) pos -= L;
                 if (pos >= L) pos -= L;                                    // rows past n_rows: harmless
-                t_tile[i] = tiles + (size_t)(1 + ub) * kGramTile;   // slot 0 = A, slot 1 + u = unit u
+                t_tile[i] = tiles + (size_t)(ub < 0 ? 0 : ub) * kGramTile;   // B unit u = slot u (A rows: unused)
                 t_row[i] = row & 127;
                 t_src[i] = xw + (size_t)pos * RW;
             }
@@ -310,11 +347,14 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
 #pragma unroll
                 for (int i = 0; i < RPT; ++i)
                     if (t_ok[i]) {
-                        if (tid + i * kGramExpWarps * 32 < 128)
-                            expand_row<false>(t_tile[i] + soff, t_row[i], wc[i]);
+                        if (tid + i * kGramExpWarps * 32 < 128)        // warps 0..3, i = 0: the A rows
+                            expand_row_tmem(tmem_base + kGramTmemA + 32u * (uint32_t)rs +
+                                                ((uint32_t)(32 * warp) << 16), wc[i]);
                         else
                             expand_row<true>(t_tile[i] + soff, t_row[i], wc[i]);
                     }
+                if (warp < 4) asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                asm volatile("tcgen05.fence::before_thread_sync;");
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&full_bar[rs]));
@@ -363,14 +403,14 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
                     if (++ms == NS) { ms = 0; mp ^= 1; }
                     asm volatile("tcgen05.fence::after_thread_sync;");
                     const uint32_t sbase = smem_u32(tiles + (size_t)s * stage_bytes);
-                    const uint64_t da = umma_desc_k128(sbase);
+                    const uint32_t ta = tmem_base + kGramTmemA + 32u * (uint32_t)s;   // A: 8 columns per K = 32
                     for (int u = 0; u < nu; u += 2) {          // two units (N = 256) per instruction where possible
-                        const uint64_t db = umma_desc_k128(sbase + (uint32_t)(1 + u) * kGramTile);
+                        const uint64_t db = umma_desc_k128(sbase + (uint32_t)u * kGramTile);
                         const uint32_t idesc = (u + 1 < nu) ? kGramIdesc256 : kGramIdesc;
 #pragma unroll
                         for (int ks = 0; ks < 4; ++ks)         // K = 32 per instruction: +32 B in the atom
-                            umma_i8(tmem_base + (uint32_t)(128 * u), da + (uint64_t)(2 * ks),
-                                    db + (uint64_t)(2 * ks), idesc, (c > c_begin || ks > 0) ? 1u : 0u);
+                            umma_i8_ts(tmem_base + (uint32_t)(128 * u), ta + (uint32_t)(8 * ks),
+                                       db + (uint64_t)(2 * ks), idesc, (c > c_begin || ks > 0) ? 1u : 0u);
                     }
                     umma_commit(smem_u32(&empty_bar[s]));      // frees the stage when the MMAs have read it
                 }
