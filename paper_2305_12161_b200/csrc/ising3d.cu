@@ -365,8 +365,7 @@ int measure_gram(ising3d *h)
     static bool attr_set = false;
     const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
     const size_t smem = ising::gram_smem_bytes(L, plan);
-    int NWB = 4;
-    if (const char *e = getenv("ISING3D_GATHER_NWB")) NWB = atoi(e);   // experiments only
+    const int NWB = 4;                         // row words per block of the x gather
     const size_t smem_x = ((size_t)64 * NWB * (L / 32 + 1) + (size_t)2 * 256 * (NWB + 1)) * 4;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(ising::gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,

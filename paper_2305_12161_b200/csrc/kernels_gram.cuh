@@ -125,17 +125,7 @@ __device__ __forceinline__ uint64_t umma_desc_k128(uint32_t saddr)
 constexpr uint32_t kGramIdesc = (2u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kGramIdesc256 = (2u << 4) | ((256u >> 3) << 17) | ((128u >> 4) << 24);   // N = 256
 
-__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc,
-                                        uint32_t accumulate)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}\n"
-        ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-
-// the same with the A operand in tensor memory (lane = row, 4 K-bytes per 32-bit column)
+// D[tmem] (+)= A[tmem] * B[smem]: A in tensor memory (lane = row, 4 K-bytes per 32-bit column)
 __device__ __forceinline__ void umma_i8_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc,
                                            uint32_t accumulate)
 {
