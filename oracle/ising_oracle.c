@@ -44,6 +44,9 @@
  *   orc_half_sweep_dcb / orc_sweep_dcb : B = L reduces to the plain 01 sweep, pure-Python
  *                         restatement on L = 8, every site proposed once (Neel read-out per
  *                         block colour), fixed points, energy monotone
+ *   orc_block_first_fine / orc_sweep_dcb_mixed : documented Philox bits, Neel read-out of the
+ *                         coarse order and of every block's fine order, pure-Python restatement,
+ *                         every site proposed once, energy monotone
  *   orc_glauber_thresholds / orc_site_uniform / orc_sweep_T : p(6-n) = 1 - p(n), p(3) = 1/2,
  *                         hand-computed thresholds, T -> infinity closed form (flip iff the top
  *                         Philox plane bit is 0), acceptance frequencies on uniform-n states
@@ -311,6 +314,58 @@ void orc_sweep_dcb(orc_t *o, uint64_t n_sweeps, int B)
         for (int coarse = 0; coarse < 2; ++coarse)
             for (int fine = 0; fine < 2; ++fine)
                 orc_half_sweep_dcb(o, o->sweep, coarse, fine, B);
+        o->sweep += 1;
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* Double checkerboard, mixed cycle (Supp. I.B PAPER.md:258; Table I    */
+/* "(mixed cycle) - double-checkerboard"): "the order of the coarse     */
+/* checkerboards (red or blue first) is chosen at random once per sweep */
+/* and the order of the fine checkerboard (lighter or darker sites      */
+/* first) is chosen at random and independently for each (red or blue)  */
+/* block and once per sweep."  Reading D15: the coarse colour updated   */
+/* first in sweep t is orc_first_colour(seed, t) (the bit of D10); the  */
+/* block with index Bi = (bz*nB + by)*nB + bx, nB = L/B, updates first  */
+/* the fine colour given by bit (Bi & 127) of Philox(key = seed,        */
+/* counter = (Bi >> 7, t, 0, tag 36)), then the other; tie bits as      */
+/* before.  Each of the two kernels of a sweep is then two masked       */
+/* passes: in every block of the coarse colour, first its first fine    */
+/* colour, then (after the barrier of step 4/6) the   */
+/* other.                                                               */
+/* ------------------------------------------------------------------ */
+int orc_block_first_fine(uint64_t seed, uint32_t t, uint32_t Bi)
+{
+    uint32_t ctr[4] = { Bi >> 7, t, 0u, 36u };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    orc_philox4x32_10(ctr, key, out);
+    return (int)((out[(Bi >> 5) & 3] >> (Bi & 31)) & 1u);
+}
+
+/* one pass: blocks of colour `coarse`; pass 0 updates each block's first fine colour, pass 1 the other */
+void orc_pass_dcb_mixed(orc_t *o, uint32_t t, int coarse, int pass, int B)
+{
+    const int L = o->L, nB = L / B;
+    #pragma omp parallel for schedule(static)
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                int bx = x / B, by = y / B, bz = z / B;
+                if (((bx + by + bz) & 1) != coarse) continue;
+                uint32_t Bi = (uint32_t)((bz * nB + by) * nB + bx);
+                int fine = orc_block_first_fine(o->seed, t, Bi) ^ pass;
+                if (((x + y + z) & 1) == fine) orc_update_site(o, x, y, z, t);
+            }
+}
+
+void orc_sweep_dcb_mixed(orc_t *o, uint64_t n_sweeps, int B)
+{
+    for (uint64_t i = 0; i < n_sweeps; ++i) {
+        int first = orc_first_colour(o->seed, o->sweep);
+        for (int k = 0; k < 2; ++k)
+            for (int pass = 0; pass < 2; ++pass)
+                orc_pass_dcb_mixed(o, o->sweep, k == 0 ? first : 1 - first, pass, B);
         o->sweep += 1;
     }
 }

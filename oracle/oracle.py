@@ -107,6 +107,12 @@ def lib():
         l.orc_half_sweep_dcb.restype = None
         l.orc_sweep_dcb.argtypes = [C.c_void_p, C.c_uint64, C.c_int]
         l.orc_sweep_dcb.restype = None
+        l.orc_block_first_fine.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32]
+        l.orc_block_first_fine.restype = C.c_int
+        l.orc_pass_dcb_mixed.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_int, C.c_int]
+        l.orc_pass_dcb_mixed.restype = None
+        l.orc_sweep_dcb_mixed.argtypes = [C.c_void_p, C.c_uint64, C.c_int]
+        l.orc_sweep_dcb_mixed.restype = None
         l.orc_glauber_thresholds.argtypes = [C.c_double, u64p]
         l.orc_glauber_thresholds.restype = None
         l.orc_site_uniform.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint32]
@@ -173,6 +179,11 @@ def radial_sums(L: int, field: np.ndarray):
     n = np.zeros(L // 2 + 1, dtype=np.uint64)
     lib().orc_radial_sums(int(L), _p(f, C.c_int64), _p(s, C.c_int64), _p(n, C.c_uint64))
     return s, n
+
+
+def block_first_fine(seed: int, t: int, block_index: int) -> int:
+    """D15: the fine colour a block updates first in sweep t (mixed-cycle double checkerboard)."""
+    return int(lib().orc_block_first_fine(int(seed), int(t), int(block_index)))
 
 
 def glauber_thresholds(T: float) -> np.ndarray:
@@ -325,6 +336,14 @@ class Oracle:
 
     def half_sweep_dcb(self, t: int, coarse: int, fine: int, block: int = 8):
         self._l.orc_half_sweep_dcb(self._h, int(t), int(coarse), int(fine), int(block))
+
+    def sweep_dcb_mixed(self, n: int = 1, block: int = 8):
+        """n sweeps of the mixed-cycle double checkerboard (Supp. I.B, D15)."""
+        assert self.L % (2 * block) == 0
+        self._l.orc_sweep_dcb_mixed(self._h, int(n), int(block))
+
+    def pass_dcb_mixed(self, t: int, coarse: int, pas: int, block: int = 8):
+        self._l.orc_pass_dcb_mixed(self._h, int(t), int(coarse), int(pas), int(block))
 
     def sweep_T(self, n: int, T: float):
         """n sweeps of finite-temperature Glauber dynamics (eq. (5), D13)."""

@@ -435,3 +435,77 @@ def test_double_checkerboard_order_readout_and_invariants():
         o.spins[...] = s0
         o.sweep_dcb(3, block=B)
         assert np.array_equal(o.spins, s0)
+
+
+# ------------------------------------------------------------------ f-2: double checkerboard, mixed cycle
+def test_dcb_mixed_bits_and_neel_readout():
+    """D15: block bits are the documented Philox bits; from the Neel state the first pass of a
+    sweep flips, in every block of the coarse colour drawn first, exactly the sites of that
+    block's first fine colour (n = 6) and nothing else: the state reads out both random choices."""
+    L, B, seed = 16, 4, 21
+    nB = L // B
+    for Bi in (0, 1, 17, 63):
+        for t in (0, 3):
+            want = (py_philox([Bi >> 7, t, 0, 36], [seed & MASK, seed >> 32])[(Bi >> 5) & 3] >> (Bi & 31)) & 1
+            assert orc.block_first_fine(seed, t, Bi) == want
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    fine = (x + y + z) & 1
+    coarse = (x // B + y // B + z // B) & 1
+    Bi = ((z // B) * nB + (y // B)) * nB + (x // B)
+    seen_first, seen_ff = set(), set()
+    for t in range(6):
+        o = orc.Oracle(L, seed, init=False)
+        o.spins[...] = inputs.neel(L)
+        first = orc.first_colour(seed, t)
+        ff = np.vectorize(lambda b: orc.block_first_fine(seed, t, int(b)))(Bi)
+        o.pass_dcb_mixed(t, first, 0, B)
+        want = inputs.neel(L).copy()
+        want[(coarse == first) & (fine == ff)] *= -1
+        assert np.array_equal(o.spins, want)
+        seen_first.add(first)
+        seen_ff |= set(np.unique(ff[coarse == first]))
+    assert seen_first == {0, 1} and seen_ff == {0, 1}
+
+
+def test_dcb_mixed_python_restatement_and_invariants():
+    from test_oracle_pins import py_site_bit
+    L, B, seed = 8, 4, 5
+    nB = L // B
+    o = orc.Oracle(L, seed)
+    s = o.spins.copy().astype(int)
+    for t in range(3):
+        first = py_philox([0, t, 0, 2], [seed & MASK, seed >> 32])[0] & 1
+        for coarse in (first, 1 - first):
+            for pas in (0, 1):
+                for z in range(L):
+                    for y in range(L):
+                        for x in range(L):
+                            if (x // B + y // B + z // B) % 2 != coarse:
+                                continue
+                            bi = ((z // B) * nB + (y // B)) * nB + (x // B)
+                            ff = (py_philox([bi >> 7, t, 0, 36], [seed & MASK, seed >> 32])[(bi >> 5) & 3] >> (bi & 31)) & 1
+                            if (x + y + z) % 2 != (ff ^ pas):
+                                continue
+                            h = (s[z][y][(x + 1) % L] + s[z][y][(x - 1) % L] + s[z][(y + 1) % L][x]
+                                 + s[z][(y - 1) % L][x] + s[(z + 1) % L][y][x] + s[(z - 1) % L][y][x])
+                            dE = 2 * s[z][y][x] * h
+                            if dE < 0 or (dE == 0 and py_site_bit(seed, L, x, y, z, t, 0)):
+                                s[z][y][x] = -s[z][y][x]
+    o.sweep_dcb_mixed(3, block=B)
+    assert np.array_equal(o.spins, s.astype(np.int8)) and o.sweep_count == 3
+    # energy never increases pass by pass; fixed points stay
+    L = 16
+    a = orc.Oracle(L, 9)
+    e = a.measure([1])[1].sum()
+    for t in range(3):
+        first = orc.first_colour(9, t)
+        for coarse in (first, 1 - first):
+            for pas in (0, 1):
+                a.pass_dcb_mixed(t, coarse, pas, 4)
+                e2 = a.measure([1])[1].sum()
+                assert e2 <= e
+                e = e2
+    a.spins[...] = inputs.slab(L, 2, 3, L // 2)
+    keep = a.spins.copy()
+    a.sweep_dcb_mixed(3, block=4)
+    assert np.array_equal(a.spins, keep)
