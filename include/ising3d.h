@@ -88,6 +88,7 @@ extern "C" {
 #define ISING3D_CYCLE_01    0   /* colour 0 then colour 1, every sweep (main text) */
 #define ISING3D_CYCLE_MIXED 1   /* first colour drawn per sweep (Supp. I.B PAPER.md:258, D10)    */
 #define ISING3D_CYCLE_DOUBLE_CB 2 /* double checkerboard, 01 cycle (Supp. I.A PAPER.md:223-240, D14) */
+#define ISING3D_CYCLE_DOUBLE_CB_MIXED 3 /* double checkerboard, mixed cycle (Supp. I.B PAPER.md:258, D15) */
 
 typedef struct ising3d ising3d_t;   /* opaque */
 
@@ -172,7 +173,12 @@ int ising3d_init_menger(ising3d_t *h, int k);
  * (coarse colour (x/8 + y/8 + z/8) mod 2); a sweep updates the red blocks (their darker sites,
  * (x+y+z) even, then their lighter sites) with everything else frozen, then the blue blocks:
  * four masked half-sweeps, every spin proposed once, tie bits as in the plain checkerboard.
- * Runs on the resident (L <= 256) and generic kernels.  Takes effect from the next sweep.
+ * Runs on the resident (L <= 256) and generic kernels.  Its mixed cycle (Table I;
+ * reading D15): the coarse colour updated first in sweep t is the D10 bit; block
+ * Bi = (bz*nB + by)*nB + bx (nB = L/8) updates first the fine colour given by bit (Bi & 127) of
+ * Philox(key = seed, counter = (Bi >> 7, t, 0, 36)), then the other; generic kernel only (the
+ * block bits of a sweep are drawn into the handle's idle state buffer).  Takes effect from the
+ * next sweep.
  * EINVAL for an unknown value, with ISING3D_VARIANT_FUSED (01 cycle only), for the double
  * checkerboard with ISING3D_VARIANT_FUSED2, or at T > 0 for anything but the 01 cycle.
  */

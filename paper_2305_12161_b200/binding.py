@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libising3d.so")
 
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
-CYCLE_01, CYCLE_MIXED, CYCLE_DOUBLE_CB = 0, 1, 2
+CYCLE_01, CYCLE_MIXED, CYCLE_DOUBLE_CB, CYCLE_DOUBLE_CB_MIXED = 0, 1, 2, 3
 MEASURE_AUTO, MEASURE_POPCOUNT, MEASURE_TENSOR = 0, 1, 2
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT = 0, 1, 2, 3, 4
 

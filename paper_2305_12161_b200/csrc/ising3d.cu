@@ -103,12 +103,13 @@ struct ising3d {
     }
     bool use_resident() const
     {
+        if (cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED) return false;   // generic kernel only
         return variant == ISING3D_VARIANT_RESIDENT ||
                (variant == ISING3D_VARIANT_AUTO && resident_ok());
     }
     bool use_fused2() const
     {
-        if (cycle == ISING3D_CYCLE_DOUBLE_CB) return false;     // four masked phases: resident / generic
+        if (cycle >= ISING3D_CYCLE_DOUBLE_CB) return false;     // masked phases: resident / generic
         return variant == ISING3D_VARIANT_FUSED2 || (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
     bool use_fused() const
@@ -217,6 +218,22 @@ int sweep_generic(ising3d *h, uint64_t n)
     const int mixed = h->cycle == ISING3D_CYCLE_MIXED;
     for (uint64_t i = 0; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
+        if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED) {
+            // D15: draw the blocks' fine orders into the idle ping-pong buffer, then for the two
+            // coarse colours in the drawn order: pass 0 (each block's first fine colour), pass 1
+            uint32_t *ff = h->state[1 - h->cur];
+            const size_t stride = h->words_per_replica();
+            const int nB = h->L / 8, n_words = nB * nB * nB / 32;
+            ising::block_order_kernel<<<dim3((unsigned)((n_words + 255) / 256), (unsigned)h->n_rep), 256, 0,
+                                        h->stream>>>(ff, stride, h->d_seeds, n_words, t);
+            for (int k = 0; k < 2; ++k)
+                for (int pass = 0; pass < 2; ++pass)
+                    for (int c = 0; c < 2; ++c)
+                        ising::halfsweep_generic_kernel<<<grid, 256, 0, h->stream>>>(
+                            h->state[h->cur], h->d_seeds, h->L, t, c, 0, k, ff, stride, pass);
+            h->launches += 7;
+            continue;
+        }
         if (h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
             // red blocks: dark sites, light sites; then the blue blocks (Supp. I.A, D14)
             for (int coarse = 0; coarse < 2; ++coarse)
@@ -480,13 +497,16 @@ int ising3d_set_temperature(ising3d_t *h, double T)
 int ising3d_set_cycle(ising3d_t *h, int cycle)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (cycle != ISING3D_CYCLE_01 && cycle != ISING3D_CYCLE_MIXED && cycle != ISING3D_CYCLE_DOUBLE_CB)
+    if (cycle < ISING3D_CYCLE_01 || cycle > ISING3D_CYCLE_DOUBLE_CB_MIXED)
         return fail(ISING3D_EINVAL, "unknown cycle");
+    if (cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && h->variant != ISING3D_VARIANT_AUTO &&
+        h->variant != ISING3D_VARIANT_GENERIC)
+        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
     if (cycle != ISING3D_CYCLE_01 && h->temperature > 0.0)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     if (cycle != ISING3D_CYCLE_01 && h->variant == ISING3D_VARIANT_FUSED)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
-    if (cycle == ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED2)
+    if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED2)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     h->cycle = cycle;
     return ISING3D_OK;
@@ -513,6 +533,9 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_RESIDENT)
         return fail(ISING3D_EINVAL, "unknown variant");
+    if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
+        variant != ISING3D_VARIANT_GENERIC)
+        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
     if (variant == ISING3D_VARIANT_FUSED2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)

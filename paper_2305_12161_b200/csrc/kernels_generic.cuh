@@ -25,6 +25,22 @@ init_spins_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ see
     reinterpret_cast<uint4 *>(state)[(size_t)rep * 2 * groups_per_colour + g] = v;
 }
 
+// Mixed-cycle double checkerboard (D15): bit Bi of ff[rep] = the fine colour block Bi updates
+// first in sweep t = bit (Bi & 127) of Philox(counter (Bi >> 7, t, 0, 36)): word wq of the bit
+// array is output word wq & 3 of the call for group wq >> 2.
+__global__ void __launch_bounds__(256)
+block_order_kernel(uint32_t *__restrict__ ff, size_t ff_stride, const uint64_t *__restrict__ seeds,
+                   int n_words, uint32_t t)
+{
+    const int wq = blockIdx.x * blockDim.x + threadIdx.x;
+    if (wq >= n_words) return;
+    const int rep = blockIdx.y;
+    const uint64_t seed = seeds[rep];
+    const uint4 r = philox4x32_10((uint32_t)(wq >> 2), t, 0u, kTagBlock, (uint32_t)seed, (uint32_t)(seed >> 32));
+    const int k = wq & 3;
+    ff[(size_t)rep * ff_stride + wq] = k == 0 ? r.x : k == 1 ? r.y : k == 2 ? r.z : r.w;
+}
+
 // `coarse` >= 0: only the sites of that coarse colour are updated (double checkerboard, D14).
 // `phase` = 0 / 1: first / second half-sweep of sweep t.  01 cycle (mixed = 0): colour = phase.
 // Mixed cycle (mixed = 1, D10): colour = phase ^ first_colour(seed of the replica, t).
@@ -79,7 +95,8 @@ init_menger_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ se
 
 __global__ void __launch_bounds__(256)
 halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds,
-                         int L, uint32_t t, int phase, int mixed, int coarse)
+                         int L, uint32_t t, int phase, int mixed, int coarse,
+                         const uint32_t *__restrict__ ff = nullptr, size_t ff_stride = 0, int pass = 0)
 {
     const int WPR = L >> 6;                                   // words per row
     const size_t WPC = (size_t)L * L * WPR;                   // words per colour
@@ -95,6 +112,7 @@ halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
     const uint32_t rho[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
     const uint4 sv = reinterpret_cast<const uint4 *>(own)[g];
     const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+    const int coarse_mixed = ff ? coarse ^ first_colour(seed, t) : 0;   // D15: k-th coarse colour of the drawn order
     uint32_t out[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -119,7 +137,17 @@ halfsweep_generic_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
             n_x = (n_same >> 1) | (next << 31);
         }
         const uint32_t upd = rule_word(s[i], rho[i], n_same, n_x, n_yp, n_ym, n_zp, n_zm);
-        const uint32_t m = dcb_mask(y, z, coarse);              // double checkerboard: one coarse colour
+        uint32_t m;
+        if (ff) {
+            // mixed-cycle double checkerboard (D15): `coarse` = 0 / 1 is the first / second coarse
+            // colour of the sweep's drawn order; the block bits come from block_order_kernel
+            const int nB = L >> 3;
+            const size_t Bi0 = ((size_t)(z >> 3) * nB + (y >> 3)) * nB + 8 * (size_t)wi;
+            const uint32_t ffbyte = (ff[(size_t)rep * ff_stride + (Bi0 >> 5)] >> (Bi0 & 31)) & 0xFFu;
+            m = dcb_mixed_mask(y, z, coarse_mixed, pass, c, ffbyte);
+        } else {
+            m = dcb_mask(y, z, coarse);                         // double checkerboard: one coarse colour
+        }
         out[i] = (upd & m) | (s[i] & ~m);
     }
     reinterpret_cast<uint4 *>(own)[g] = make_uint4(out[0], out[1], out[2], out[3]);

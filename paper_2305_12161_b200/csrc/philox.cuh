@@ -80,6 +80,8 @@ constexpr uint32_t kTagTie = 0u;       // tie bits of sweep t:          counter 
 constexpr uint32_t kTagInit = 1u;      // T = infinity start:           counter (q, 0, colour, 1)
 constexpr uint32_t kTagOrder = 2u;     // mixed cycle, first colour:    counter (0, t, 0, 2), word 0 bit 0
 constexpr uint32_t kTagMenger = 3u;    // Menger start, tile sign bits: counter (T >> 7, k, 0, 3)
+constexpr uint32_t kTagBlock = 36u;    // mixed double checkerboard, per-block fine order: (Bi >> 7, t, 0, 36)
+                                       // (tags 4..35: bit planes of the finite-T uniforms, D13)
 
 // Mixed cycle (Supp. I.B PAPER.md:258, D10): the colour updated first in sweep t.
 __host__ __device__ __forceinline__ int first_colour(uint64_t seed, uint32_t t)
@@ -97,6 +99,21 @@ __device__ __forceinline__ uint32_t dcb_mask(int y, int z, int coarse)
 {
     if (coarse < 0) return 0xFFFFFFFFu;
     return (((y >> 3) + (z >> 3) + coarse) & 1) ? 0xF0F0F0F0u : 0x0F0F0F0Fu;
+}
+
+// Mixed-cycle double checkerboard (D15): `ffbyte` holds the first-fine-colour bits of the 8
+// blocks a packed word spans (bit b = block bx = 8 wi + b).  In pass `pass` of coarse colour
+// `coarse`, the colour-c sites of the word that are updated are those of the blocks with
+// parity == coarse and (bit ^ pass) == c.
+__device__ __forceinline__ uint32_t dcb_mixed_mask(int y, int z, int coarse, int pass, int c, uint32_t ffbyte)
+{
+    const uint32_t want = (c ^ pass) ? ffbyte : ~ffbyte;                       // bit == c ^ pass
+    const uint32_t par = (((y >> 3) + (z >> 3) + coarse) & 1) ? 0xAAu : 0x55u;   // block parity == coarse
+    uint32_t x = want & par & 0xFFu;                                           // bit b -> nibble b
+    x = (x | (x << 12)) & 0x000F000Fu;
+    x = (x | (x << 6)) & 0x03030303u;
+    x = (x | (x << 3)) & 0x11111111u;
+    return x * 0xFu;
 }
 
 // ---------------------------------------------------------------------------

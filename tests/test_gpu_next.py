@@ -363,3 +363,39 @@ def test_double_checkerboard_batch_neel_and_errors(B, orc):
     with pytest.raises(B.Ising3DError):
         sim.set_temperature(2.0)
     sim.free()
+
+
+@pytest.mark.parametrize("L,seed,cps", [(64, 1, [1, 2, 6]), (128, 7, [1, 4]), (192, 8, [2]), (512, 11, [1, 2])])
+def test_double_checkerboard_mixed_against_oracle(B, orc, L, seed, cps):
+    sim = B.Ising3D(L, [seed])
+    sim.set_cycle(B.CYCLE_DOUBLE_CB_MIXED)
+    assert sim.variant_name == "generic"
+    ref = orc.Oracle(L, seed)
+    t = 0
+    for cp in cps:
+        sim.sweep(cp - t)
+        ref.sweep_dcb_mixed(cp - t, block=8)
+        t = cp
+        assert np.array_equal(sim.get_state(), ref.export_words()), "state differs at sweep %d" % cp
+    if L <= 192:
+        check_measure(sim.measure(), ref.measure_full())
+    sim.set_cycle(B.CYCLE_01)
+    sim.sweep(1)
+    ref.sweep(1)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    sim.free()
+
+
+def test_double_checkerboard_mixed_batch_and_errors(B, orc):
+    L, seeds = 64, [100, 101, 163]
+    batch = B.Ising3D(L, seeds)
+    batch.set_cycle(B.CYCLE_DOUBLE_CB_MIXED)
+    batch.sweep(4)
+    st = batch.get_state().reshape(3, -1)
+    for i, s in enumerate(seeds):
+        ref = orc.Oracle(L, s)
+        ref.sweep_dcb_mixed(4, block=8)
+        assert np.array_equal(st[i], ref.export_words())
+    with pytest.raises(B.Ising3DError):
+        batch.set_variant(B.VARIANT_RESIDENT)
+    batch.free()
