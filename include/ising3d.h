@@ -249,6 +249,10 @@ typedef struct {
 } ising3d_radial_t;
 int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out);
 
+/* Give back the device memory and cuFFT plans ising3d_measure_radial keeps between calls
+ * (8 bytes per site + work area: 128 GiB at L = 2048).  The next call re-creates them. */
+int ising3d_release_radial(ising3d_t *h);
+
 /*
  * Copy the canonical packed state (D3) to / from HOST memory.
  * n_words must equal n_rep * L^3/32.  Both synchronise the stream.

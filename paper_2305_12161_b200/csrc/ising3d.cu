@@ -695,6 +695,23 @@ int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out)
     return ISING3D_OK;
 }
 
+int ising3d_release_radial(ising3d_t *h)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    cudaStreamSynchronize(h->stream);
+    if (h->plan_fwd) cufftDestroy(h->plan_fwd);
+    if (h->plan_inv) cufftDestroy(h->plan_inv);
+    if (h->fft_buf) cudaFree(h->fft_buf);
+    if (h->fft_work) cudaFree(h->fft_work);
+    if (h->d_rad) cudaFree(h->d_rad);
+    h->plan_fwd = h->plan_inv = 0;
+    h->fft_buf = nullptr;
+    h->fft_work = nullptr;
+    h->d_rad = nullptr;
+    h->fft_ready = false;
+    return ISING3D_OK;
+}
+
 int ising3d_get_state(ising3d_t *h, uint32_t *words, size_t n_words, uint64_t *sweep)
 {
     if (!h || !words) return fail(ISING3D_EINVAL, "null pointer");
@@ -774,11 +791,7 @@ void ising3d_free(ising3d_t *h)
 {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
-    if (h->plan_fwd) cufftDestroy(h->plan_fwd);
-    if (h->plan_inv) cufftDestroy(h->plan_inv);
-    if (h->fft_buf) cudaFree(h->fft_buf);
-    if (h->fft_work) cudaFree(h->fft_work);
-    if (h->d_rad) cudaFree(h->d_rad);
+    ising3d_release_radial(h);
     if (h->owns_mem && h->base) cudaFree(h->base);
     delete h;
 }

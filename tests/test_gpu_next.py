@@ -255,6 +255,12 @@ def test_radial_estimator_large_identities(B):
     # the radial C and the axis-averaged C agree to a few per cent at short distance
     assert abs(r["C_rad"][0][1] - m["C"][0][1]) < 0.1
     assert abs(r["ell"][0] - m["ell"][0]) < 0.25 * m["ell"][0]
+    import torch
+    free0 = torch.cuda.mem_get_info()[0]
+    sim.release_radial()                               # 8.6 GB field + work area go back
+    assert torch.cuda.mem_get_info()[0] > free0 + 8 * 2 ** 30
+    r2 = sim.measure_radial()                          # and are re-created on demand
+    assert np.array_equal(r2["corr_sum"], r["corr_sum"])
     sim.free()
 
 
