@@ -29,7 +29,10 @@
 
 namespace ising {
 
-constexpr int kF2Stages = 4;     // shared-memory ring depth S; prefetch distance S-1
+#ifndef ISING_F2_STAGES
+#define ISING_F2_STAGES 4
+#endif
+constexpr int kF2Stages = ISING_F2_STAGES;     // shared-memory ring depth S; prefetch distance S-1
 
 // Per-launch Philox constants (host-folded, D5): counter (q, t, colour, 0), key (k0, k1).
 struct SweepConsts {
@@ -151,11 +154,11 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
 {
     constexpr int S = kF2Stages;
     constexpr int M = PH % 3, Z = (PH + 1) % 3, P = (PH + 2) % 3;
-    const int s = k & (S - 1);
+    const int s = k % S;
     mbar_wait(smem_u32(&c.bars[s]), (uint32_t)((k / S) & 1));
     const uint4 *Wnew = c.Wst + s * PLANE;
     const uint4 *Bold = c.Bst + s * PLANE;
-    const uint4 *Wz = c.Wst + ((k - 1) & (S - 1)) * PLANE;       // plane z of W_old
+    const uint4 *Wz = c.Wst + ((k + S - 1) % S) * PLANE;          // plane z of W_old
     w.W[P][0] = Wnew[c.si0];
     w.W[P][1] = Wnew[c.si0 + R4];
     const uint4 Bo0 = Bold[c.si0], Bo1 = Bold[c.si0 + R4];
@@ -273,7 +276,7 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     const uint4 *pgw = srcW + (size_t)pzw * plane_u4;
     const uint4 *pgb = srcB + (size_t)pzb * plane_u4;
     auto issue_next = [&]() {
-        const int s = pk & (S - 1);
+        const int s = pk % S;
         const uint32_t bar = smem_u32(&bars[s]);
         mbar_expect_tx(bar, 2u * (uint32_t)PLANE * 16u);
         bulk_g2s(smem_u32(Wst + s * PLANE), pgw + (size_t)ybase * R4, bytes1, bar);
