@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=2048)
     ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (throughput window)")
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "fused3"])
     ap.add_argument("--ref-L", type=int, default=512, help="--impl reference: lattice size of the CPU sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -230,7 +230,8 @@ def run_ours(args):
     L, S = args.L, args.sweeps
     seed = rank_seed(rank)
     variant = {"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
-               "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2}[args.variant]
+               "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2,
+               "fused3": binding.VARIANT_FUSED3}[args.variant]
     sim = binding.Ising3D(L, [seed], variant=variant)
     N = L ** 3
     n_words = N // 32
@@ -308,9 +309,10 @@ def run_ours(args):
 
     # ---------------- roofline of the dominant kernel (the sweep kernel) ----------------
     peak, peak_src, peaks = measured_peak()
-    kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel"}.get(
-        sim.variant_name, "halfsweep_generic_kernel")
-    launches_per_sweep = 1 if sim.variant_name in ("fused", "fused2") else 2
+    kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel",
+              "fused3": "fused3_sweep2_kernel"}.get(sim.variant_name, "halfsweep_generic_kernel")
+    # fused3: one launch = two sweeps (an odd last sweep of a step runs on fused2; S is even here)
+    launches_per_sweep = {"fused": 1, "fused2": 1, "fused3": 0.5}.get(sim.variant_name, 2)
     avg_launch_ms = sweep_ms / (S * launches_per_sweep)
     algo_bytes_per_launch = ALGO_BYTES_PER_SITE_UPDATE * N / launches_per_sweep
     achieved = algo_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
@@ -331,7 +333,7 @@ def run_ours(args):
         "frac_of_min_roofline": (N * S / (sweep_ms * 1e6)) / min(hbm_bound, alu_bound),
         # the stricter view: the N/4 bytes per sweep a fused black+white pass cannot avoid moving
         "frac_on_fused_floor_bytes": (0.25 * N / launches_per_sweep / (avg_launch_ms * 1e-3) / 1e9) / peak
-        if launches_per_sweep == 1 else None,
+        if launches_per_sweep <= 1 else None,
         "note": "algorithmic bytes = 3N/8 per sweep (two half-sweeps each read both colours' "
                 "share and write one); the fused kernel moves ~N/4 + halo, so frac can pass 1",
     }

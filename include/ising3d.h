@@ -78,6 +78,9 @@ extern "C" {
 #define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096)        */
 #define ISING3D_VARIANT_RESIDENT 4  /* lattice resident in the shared memory of a thread-block
                                        cluster, all sweeps of a call in one launch (L in 64..256) */
+#define ISING3D_VARIANT_FUSED3  5   /* two sweeps per launch, the state in between stays in shared
+                                       memory (L in {1024, 2048}, 01 cycle); an odd last sweep and
+                                       the mixed cycle run on fused2                           */
 
 /* measurement kernels (ising3d_set_measure_variant) */
 #define ISING3D_MEASURE_AUTO     0  /* tensor where the shape allows (L % 512 == 0), else popcount */

@@ -20,6 +20,7 @@ OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 CYCLE_01, CYCLE_MIXED, CYCLE_DOUBLE_CB, CYCLE_DOUBLE_CB_MIXED = 0, 1, 2, 3
 MEASURE_AUTO, MEASURE_POPCOUNT, MEASURE_TENSOR = 0, 1, 2
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT = 0, 1, 2, 3, 4
+VARIANT_FUSED3 = 5
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",

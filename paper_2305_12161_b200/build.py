@@ -28,7 +28,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             and os.path.getmtime(LIB) >= max(os.path.getmtime(s) for s in srcs)):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = ["nvcc"] + NVCC_FLAGS + ["-o", tmp, os.path.join(CSRC, "ising3d.cu")]
+    # ISING3D_NVCC_EXTRA: extra nvcc arguments (e.g. "-DISING_F2_STAGES=5") for kernel experiments
+    extra = os.environ.get("ISING3D_NVCC_EXTRA", "").split()
+    cmd = ["nvcc"] + NVCC_FLAGS + extra + ["-o", tmp, os.path.join(CSRC, "ising3d.cu")]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

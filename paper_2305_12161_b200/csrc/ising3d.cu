@@ -16,6 +16,7 @@
 
 #include "kernels_fused.cuh"
 #include "kernels_fused2.cuh"
+#include "kernels_fused3.cuh"
 #include "kernels_generic.cuh"
 #include "kernels_fft.cuh"
 #include "kernels_gram.cuh"
@@ -107,10 +108,13 @@ struct ising3d {
         return variant == ISING3D_VARIANT_RESIDENT ||
                (variant == ISING3D_VARIANT_AUTO && resident_ok());
     }
+    bool fused3_ok() const { return n_rep == 1 && ising::fused3_supported(L); }
+    bool use_fused3() const { return variant == ISING3D_VARIANT_FUSED3 && cycle == ISING3D_CYCLE_01; }
     bool use_fused2() const
     {
         if (cycle >= ISING3D_CYCLE_DOUBLE_CB) return false;     // masked phases: resident / generic
-        return variant == ISING3D_VARIANT_FUSED2 || (variant == ISING3D_VARIANT_AUTO && fused2_ok());
+        return variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3 ||
+               (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
     bool use_fused() const
     {
@@ -283,7 +287,18 @@ int sweep_resident(ising3d *h, uint64_t n)
 int sweep_fused(ising3d *h, uint64_t n, bool gen2)
 {
     const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
-    for (uint64_t i = 0; i < n; ++i) {
+    uint64_t i = 0;
+    // pairs of sweeps with the intermediate state on chip (01 cycle); an odd last sweep below
+    for (; gen2 && h->use_fused3() && i + 2 <= n; i += 2) {
+        cudaError_t e = ising::launch_fused3_sweep2(h->state[h->cur], h->state[1 - h->cur], h->L,
+                                                    (uint32_t)(h->sweep + i), h->seeds[0],
+                                                    h->sm_count, h->stream);
+        if (e != cudaSuccess)
+            return fail(ISING3D_ECUDA, std::string("fused3 sweep launch: ") + cudaGetErrorString(e));
+        h->cur = 1 - h->cur;
+        h->launches += 1;
+    }
+    for (; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
         // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
         const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(h->seeds[0], t) : 0;
@@ -506,7 +521,8 @@ int ising3d_set_cycle(ising3d_t *h, int cycle)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     if (cycle != ISING3D_CYCLE_01 && h->variant == ISING3D_VARIANT_FUSED)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
-    if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED2)
+    if (cycle >= ISING3D_CYCLE_DOUBLE_CB &&
+        (h->variant == ISING3D_VARIANT_FUSED2 || h->variant == ISING3D_VARIANT_FUSED3))
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     h->cycle = cycle;
     return ISING3D_OK;
@@ -531,12 +547,13 @@ int ising3d_init_menger(ising3d_t *h, int k)
 int ising3d_set_variant(ising3d_t *h, int variant)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_RESIDENT)
+    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED3)
         return fail(ISING3D_EINVAL, "unknown variant");
     if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
         variant != ISING3D_VARIANT_GENERIC)
         return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
-    if (variant == ISING3D_VARIANT_FUSED2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB)
+    if ((variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3) &&
+        h->cycle == ISING3D_CYCLE_DOUBLE_CB)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
@@ -544,6 +561,8 @@ int ising3d_set_variant(ising3d_t *h, int variant)
         return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())
         return fail(ISING3D_EINVAL, "fused2 kernel needs n_rep == 1 and L in {512,1024,2048,4096}");
+    if (variant == ISING3D_VARIANT_FUSED3 && !h->fused3_ok())
+        return fail(ISING3D_EINVAL, "fused3 kernel needs n_rep == 1 and L in {1024,2048}");
     if (variant == ISING3D_VARIANT_RESIDENT && !h->resident_ok())
         return fail(ISING3D_EINVAL, "resident kernel needs L in {64,128,256} and a cluster that fits");
     h->variant = variant;
@@ -772,7 +791,7 @@ const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";
     if (h->temperature > 0.0) return "glauber";
-    return h->use_resident() ? "resident" : h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
+    return h->use_resident() ? "resident" : h->use_fused3() ? "fused3" : h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
 }
 
 int ising3d_cluster_size(const ising3d_t *h)

@@ -46,6 +46,7 @@ def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto")
         times.append(n_total)
     sim = binding.Ising3D(L, seeds, variant={"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
                                              "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2,
+                                             "fused3": binding.VARIANT_FUSED3,
                                              "resident": binding.VARIANT_RESIDENT}[variant])
     N = L ** 3 * len(seeds)
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -92,7 +93,7 @@ def main(argv=None):
     ap.add_argument("--configs", default=",".join(inputs.WORKLOADS))
     ap.add_argument("--max-sweeps", type=int, default=None,
                     help="truncate each workload to this many sweeps (default: the full run)")
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "resident"],
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "fused3", "resident"],
                     help="sweep kernel (default: the library's choice)")
     ap.add_argument("--out", default=None, help="also append the JSON lines to this file")
     args = ap.parse_args(argv)

@@ -32,7 +32,7 @@ def orc():
 
 def VARIANTS(B):
     return {"auto": B.VARIANT_AUTO, "generic": B.VARIANT_GENERIC, "fused": B.VARIANT_FUSED,
-            "fused2": B.VARIANT_FUSED2, "resident": B.VARIANT_RESIDENT}
+            "fused2": B.VARIANT_FUSED2, "resident": B.VARIANT_RESIDENT, "fused3": B.VARIANT_FUSED3}
 
 
 def check_measure(got, want, rep=0):
@@ -144,7 +144,8 @@ def test_fused_kernel_larger_L(B, orc, L, seed, cps, variant):
 
 
 @pytest.mark.parametrize("L,variant", [(256, "fused"), (512, "fused"), (1024, "fused"), (2048, "fused"),
-                                       (512, "fused2"), (1024, "fused2"), (2048, "fused2")])
+                                       (512, "fused2"), (1024, "fused2"), (2048, "fused2"),
+                                       (1024, "fused3"), (2048, "fused3")])
 def test_fused_equals_generic(B, L, variant):
     """Not an oracle check: the kernels must agree bit for bit (also at sizes and times
     the oracle cannot reach); the generic kernel is oracle-checked above."""
@@ -157,6 +158,30 @@ def test_fused_equals_generic(B, L, variant):
         assert np.array_equal(a.get_state(), b.get_state())
     a.free()
     b.free()
+
+
+def test_fused3_against_oracle(B, orc):
+    """Two sweeps per launch (the state in between never leaves the SM): pairs, an odd tail on
+    fused2, and pairs starting at odd t, against the oracle."""
+    thin = np.array([0, 1, 2, 3, 7, 64, 255, 256, 511, 512], dtype=np.int32)
+    run_against_oracle(B, orc, 1024, 3, [2, 3, 7, 8], B.VARIANT_FUSED3, measure_at={8}, thin_r=thin)
+
+
+def test_fused3_full_size_sampled_sites(B, orc):
+    """L = 2048, one launch = sweeps 0 and 1: sampled sites (tile borders of the 56-row tiles, odd
+    chunk borders, wraps) against the oracle's light-cone recursion."""
+    L, seed = 2048, 4
+    sim = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED3)
+    assert sim.variant_name == "fused3"
+    xyz = _sample_sites(L, 3000, 23, RPT=56)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    sim.sweep(2)
+    assert sim.launch_count == 2                     # init + one launch for two sweeps
+    got = _bits_at(sim.get_state(buf), L, xyz)
+    want = orc.sites_after(seed, L, xyz, 4)
+    bad = np.nonzero(got != want)[0]
+    assert bad.size == 0, "%d sampled sites differ, first %s" % (bad.size, xyz[bad[:5]].tolist())
+    sim.free()
 
 
 # ------------------------------------------------------------------ config 5 (full size, sampled)
