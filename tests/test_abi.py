@@ -33,6 +33,16 @@ def test_header_symbols_are_exported(lib):
     assert sorted(binding.EXPORTED) == names
 
 
+def test_binding_constants_match_the_header():
+    """Every ISING3D_* integer constant of the header has the same value in the binding."""
+    from paper_2305_12161_b200 import binding
+    src = open(os.path.join(ROOT, "include", "ising3d.h")).read()
+    defs = dict(re.findall(r"#define\s+ISING3D_([A-Z0-9_]+)\s+\(?(-?\d+)\)?", src))
+    assert len(defs) >= 17
+    for name, val in defs.items():
+        assert getattr(binding, name) == int(val), name
+
+
 def test_library_is_sm100a_and_uses_bulk_async_copies():
     import shutil
     import subprocess
