@@ -3,7 +3,7 @@
 the trajectory of the measured quantities and the throughput in site-updates/ns.
 
   python -m paper_2305_12161_b200.run_configs [--configs config1_L64,config5_L2048]
-         [--max-sweeps N] [--out results.jsonl]
+         [--max-sweeps N] [--radial] [--out results.jsonl]
 
 Per workload: ising3d_init(_batch) from the workload's seeds, then for
 each measurement time T(n) (S12): ising3d_sweep(dt), ising3d_measure().  Reported:
@@ -34,7 +34,7 @@ def ell_from_C(C: np.ndarray, c: float = 0.5) -> float:
     return float("nan")
 
 
-def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto"):
+def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto", radial: bool = False):
     import torch
     from . import binding
 
@@ -50,7 +50,7 @@ def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto")
                                              "resident": binding.VARIANT_RESIDENT}[variant])
     N = L ** 3 * len(seeds)
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    t_sweeps = t_meas = 0.0
+    t_sweeps = t_meas = t_rad = 0.0
     t = 0
     e_all0 = ev(); e_all0.record()
     for cp in times:
@@ -72,10 +72,19 @@ def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto")
                 "ell_nan": int(np.isnan(m["ell"]).sum())}
         if len(seeds) > 1:
             line["ell_of_mean_C"] = ell_from_C(m["C"].mean(axis=0))
+        if radial:      # the paper's estimator (eq. 7 + radial average), outside the timed totals
+            e3, e4 = ev(), ev()
+            e3.record()
+            r = sim.measure_radial()
+            e4.record()
+            torch.cuda.synchronize()
+            line["ell_radial_mean"] = float(np.nanmean(r["ell"])) if np.isfinite(r["ell"]).any() else None
+            line["ms_measure_radial"] = e3.elapsed_time(e4)
+            t_rad += line["ms_measure_radial"]
         emit(line)
         t = cp
     e_all1 = ev(); e_all1.record(); torch.cuda.synchronize()
-    total_ms = e_all0.elapsed_time(e_all1)
+    total_ms = e_all0.elapsed_time(e_all1) - t_rad
     summary = {"workload": name, "summary": True, "L": L, "replicas": len(seeds), "sweeps": n_total,
                "checkpoints": len(times), "kernel": sim.variant_name, "cluster_size": sim.cluster_size,
                "site_updates_per_ns_sweeps": N * n_total / (t_sweeps * 1e6),
@@ -95,6 +104,8 @@ def main(argv=None):
                     help="truncate each workload to this many sweeps (default: the full run)")
     ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "fused3", "resident"],
                     help="sweep kernel (default: the library's choice)")
+    ap.add_argument("--radial", action="store_true",
+                    help="also call ising3d_measure_radial (FFT + radial average) at every checkpoint")
     ap.add_argument("--out", default=None, help="also append the JSON lines to this file")
     args = ap.parse_args(argv)
     from . import build
@@ -109,7 +120,7 @@ def main(argv=None):
             fh.flush()
 
     for name in args.configs.split(","):
-        run_workload(name.strip(), args.max_sweeps, emit, args.variant)
+        run_workload(name.strip(), args.max_sweeps, emit, args.variant, args.radial)
     return 0
 
 
