@@ -122,7 +122,9 @@ size_t ising3d_words_per_replica(int L);
  * Create one lattice in the T = infinity start of `seed` (D6), sweep = 0.
  * PAPER.md:45.  *h is written only on success.  Runs on the legacy default
  * stream until ising3d_set_stream is called; the handle is created on the
- * CUDA device current at the time of the call.
+ * CUDA device current at the time of the call, and every later call on it
+ * must be made with that device current (handles on several devices may
+ * live in one process).
  */
 int ising3d_init(ising3d_t **h, int L, uint64_t seed);
 

@@ -394,17 +394,20 @@ int fft_setup(ising3d *h)
 int measure_gram(ising3d *h)
 {
     const int L = h->L, nr = L / 2 + 1, cpr = h->counts_per_replica();
-    static bool attr_set = false;
+    static unsigned long long attr_set = 0;     // bit per device: function attributes are per device
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    const unsigned long long dev_bit = 1ull << (dev & 63);
     const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
     const size_t smem = ising::gram_smem_bytes(L, plan);
     const int NWB = 4;                         // row words per block of the x gather
     const size_t smem_x = ((size_t)64 * NWB * (L / 32 + 1) + (size_t)2 * 256 * (NWB + 1)) * 4;
-    if (!attr_set) {
+    if (!(attr_set & dev_bit)) {
         CUDA_TRY(cudaFuncSetAttribute(ising::gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       210 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(ising::gather_lines_x_kernel,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-        attr_set = true;
+        attr_set |= dev_bit;
     }
     CUDA_TRY(cudaMemsetAsync(h->d_gsum, 0, (size_t)h->n_rep * 3 * nr * 8, h->stream));
     CUDA_TRY(cudaMemsetAsync(h->d_queue, 0, (size_t)h->n_rep * 3 * 4, h->stream));
@@ -610,8 +613,11 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
         const int C = ising::autocorr_tile_sequences(L);
         const int n_tiles = (L * L / 32) / C;
         const size_t smem = ising::autocorr_smem_bytes(L, C);
-        static bool attr_set = false;
-        if (!attr_set) {
+        static unsigned long long attr_set = 0;     // bit per device
+        int dev = 0;
+        CUDA_TRY(cudaGetDevice(&dev));
+        const unsigned long long dev_bit = 1ull << (dev & 63);
+        if (!(attr_set & dev_bit)) {
             const int max_smem = (int)ising::autocorr_smem_bytes(4096, 8) + 4096;
             CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<0>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
@@ -619,7 +625,7 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
             CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<2>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-            attr_set = true;
+            attr_set |= dev_bit;
         }
         int gx = std::max(1, (h->sm_count + h->n_rep - 1) / h->n_rep);
         gx = std::min(gx, n_tiles);

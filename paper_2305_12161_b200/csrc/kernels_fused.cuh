@@ -254,8 +254,10 @@ inline cudaError_t launch_fused_t(const uint32_t *src, uint32_t *dst, int L, uin
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kFusedStages + 2) + kFusedStages * 8;
     static FusedPlan plan = {0, 0, 0, 0};
-    static int plan_L = 0, plan_sms = 0;
-    if (plan_L != L || plan_sms != sm_count) {
+    static int plan_L = 0, plan_sms = 0, plan_dev = -1;   // attributes are per device
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
         cudaError_t e = cudaFuncSetAttribute(fused_sweep_kernel<R4, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -273,6 +275,7 @@ inline cudaError_t launch_fused_t(const uint32_t *src, uint32_t *dst, int L, uin
         plan.smem = smem;
         plan_L = L;
         plan_sms = sm_count;
+        plan_dev = dev;
     }
     dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
     fused_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(

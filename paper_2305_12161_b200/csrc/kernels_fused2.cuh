@@ -338,8 +338,11 @@ inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, in
     constexpr int TY = 2 * NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
-    static int plan_L = 0, plan_sms = 0, nty = 0, RPT = 0, nzc = 0;
-    if (plan_L != L || plan_sms != sm_count) {
+    // function attributes are per device: the plan is keyed on the current device as well
+    static int plan_L = 0, plan_sms = 0, plan_dev = -1, nty = 0, RPT = 0, nzc = 0;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
         cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -357,6 +360,7 @@ inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, in
         if (nzc > L / 8) nzc = L / 8;
         plan_L = L;
         plan_sms = sm_count;
+        plan_dev = dev;
     }
     dim3 grid((unsigned)nty, (unsigned)nzc);
     fused2_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(

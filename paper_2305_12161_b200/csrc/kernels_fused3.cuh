@@ -333,8 +333,11 @@ inline cudaError_t launch_fused3_t(const uint32_t *src, uint32_t *dst, int L, co
     constexpr int PLANE = TY * R4;
     constexpr size_t smem =
         (size_t)PLANE * 16 * (2 * kF3Stages + 2 * kF3Mid + 2) + kF3Stages * 8 + 16;
-    static int plan_L = 0, plan_sms = 0, nty = 0, RPT = 0, nzc = 0;
-    if (plan_L != L || plan_sms != sm_count) {
+    // function attributes are per device: the plan is keyed on the current device as well
+    static int plan_L = 0, plan_sms = 0, plan_dev = -1, nty = 0, RPT = 0, nzc = 0;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
         cudaError_t e = cudaFuncSetAttribute(fused3_sweep2_kernel<R4, NT>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -348,6 +351,7 @@ inline cudaError_t launch_fused3_t(const uint32_t *src, uint32_t *dst, int L, co
         if (nzc > L / 16) nzc = L / 16;
         plan_L = L;
         plan_sms = sm_count;
+        plan_dev = dev;
     }
     dim3 grid((unsigned)nty, (unsigned)nzc);
     fused3_sweep2_kernel<R4, NT><<<grid, 2 * NT, smem, stream>>>(
