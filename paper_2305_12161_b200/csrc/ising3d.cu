@@ -80,8 +80,8 @@ struct ising3d {
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
     int counts_per_replica() const { return 1 + 3 * (L / 2 + 1); }
-    bool fused_ok() const { return n_rep == 1 && ising::fused_supported(L); }
-    bool fused2_ok() const { return n_rep == 1 && ising::fused2_supported(L); }
+    bool fused_ok() const { return ising::fused_supported(L); }
+    bool fused2_ok() const { return ising::fused2_supported(L); }
     bool use_gram() const
     {
         return measure_variant == ISING3D_MEASURE_TENSOR ||
@@ -108,7 +108,7 @@ struct ising3d {
         return variant == ISING3D_VARIANT_RESIDENT ||
                (variant == ISING3D_VARIANT_AUTO && resident_ok());
     }
-    bool fused3_ok() const { return n_rep == 1 && ising::fused3_supported(L); }
+    bool fused3_ok() const { return ising::fused3_supported(L); }
     bool use_fused3() const { return variant == ISING3D_VARIANT_FUSED3 && cycle == ISING3D_CYCLE_01; }
     bool use_fused2() const
     {
@@ -284,33 +284,41 @@ int sweep_resident(ising3d *h, uint64_t n)
     return ISING3D_OK;
 }
 
+// One launch per replica and sweep (pair of sweeps for fused3): the replicas of a batch are
+// independent lattices at a stride of words_per_replica() in both ping-pong buffers.
 int sweep_fused(ising3d *h, uint64_t n, bool gen2)
 {
-    const ising::PhiloxKeys keys = ising::make_philox_keys(h->seeds[0]);
+    const size_t wpr = h->words_per_replica();
     uint64_t i = 0;
     // pairs of sweeps with the intermediate state on chip (01 cycle); an odd last sweep below
     for (; gen2 && h->use_fused3() && i + 2 <= n; i += 2) {
-        cudaError_t e = ising::launch_fused3_sweep2(h->state[h->cur], h->state[1 - h->cur], h->L,
-                                                    (uint32_t)(h->sweep + i), h->seeds[0],
-                                                    h->sm_count, h->stream);
-        if (e != cudaSuccess)
-            return fail(ISING3D_ECUDA, std::string("fused3 sweep launch: ") + cudaGetErrorString(e));
+        for (int rep = 0; rep < h->n_rep; ++rep) {
+            cudaError_t e = ising::launch_fused3_sweep2(
+                h->state[h->cur] + rep * wpr, h->state[1 - h->cur] + rep * wpr, h->L,
+                (uint32_t)(h->sweep + i), h->seeds[rep], h->sm_count, h->stream);
+            if (e != cudaSuccess)
+                return fail(ISING3D_ECUDA, std::string("fused3 sweep launch: ") + cudaGetErrorString(e));
+        }
         h->cur = 1 - h->cur;
-        h->launches += 1;
+        h->launches += h->n_rep;
     }
     for (; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i);
-        // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
-        const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(h->seeds[0], t) : 0;
-        cudaError_t e =
-            gen2 ? ising::launch_fused2_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t,
-                                              h->seeds[0], first, h->sm_count, h->stream)
-                 : ising::launch_fused_sweep(h->state[h->cur], h->state[1 - h->cur], h->L, t, keys,
-                                             h->sm_count, h->stream);
-        if (e != cudaSuccess)
-            return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
+        for (int rep = 0; rep < h->n_rep; ++rep) {
+            const uint64_t seed = h->seeds[rep];
+            const uint32_t *src = h->state[h->cur] + rep * wpr;
+            uint32_t *dst = h->state[1 - h->cur] + rep * wpr;
+            // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
+            const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
+            cudaError_t e =
+                gen2 ? ising::launch_fused2_sweep(src, dst, h->L, t, seed, first, h->sm_count, h->stream)
+                     : ising::launch_fused_sweep(src, dst, h->L, t, ising::make_philox_keys(seed),
+                                                 h->sm_count, h->stream);
+            if (e != cudaSuccess)
+                return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
+        }
         h->cur = 1 - h->cur;
-        h->launches += 1;
+        h->launches += h->n_rep;
     }
     CUDA_TRY(cudaGetLastError());
     return ISING3D_OK;
@@ -561,11 +569,11 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
-        return fail(ISING3D_EINVAL, "fused kernel needs n_rep == 1 and L in {256,512,1024,2048,4096}");
+        return fail(ISING3D_EINVAL, "fused kernel needs L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())
-        return fail(ISING3D_EINVAL, "fused2 kernel needs n_rep == 1 and L in {512,1024,2048,4096}");
+        return fail(ISING3D_EINVAL, "fused2 kernel needs L in {512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED3 && !h->fused3_ok())
-        return fail(ISING3D_EINVAL, "fused3 kernel needs n_rep == 1 and L in {1024,2048}");
+        return fail(ISING3D_EINVAL, "fused3 kernel needs L in {1024,2048}");
     if (variant == ISING3D_VARIANT_RESIDENT && !h->resident_ok())
         return fail(ISING3D_EINVAL, "resident kernel needs L in {64,128,256} and a cluster that fits");
     h->variant = variant;

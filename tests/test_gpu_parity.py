@@ -304,6 +304,46 @@ def test_config3_batch_equals_singles_and_oracle(B, orc, variant):
         one.free()
 
 
+@pytest.mark.parametrize("L,variant,name", [(512, "auto", "fused2"), (1024, "fused3", "fused3"),
+                                            (256, "fused", "fused")])
+def test_large_L_batch_equals_singles(B, orc, L, variant, name):
+    """Batches at the sizes of the fused kernels: one launch per replica and sweep, each replica
+    bit-identical to a single-lattice handle with its seed; the mixed cycle draws
+    its first colour per replica.  The first replica also against the oracle at L <= 512."""
+    seeds = [21, 22, 23]
+    batch = B.Ising3D(L, seeds, variant=VARIANTS(B)[variant])
+    assert batch.variant_name == name and batch.n_rep == 3
+    singles = [B.Ising3D(L, [s], variant=B.VARIANT_GENERIC) for s in seeds]
+    wpr = L ** 3 // 32
+    for n in (1, 2, 3):
+        batch.sweep(n)
+        st = batch.get_state().reshape(3, wpr)
+        for i, one in enumerate(singles):
+            one.sweep(n)
+            assert np.array_equal(st[i], one.get_state())
+    mb = batch.measure()
+    for i, one in enumerate(singles):
+        m1 = one.measure()
+        assert int(mb["n_up"][i]) == int(m1["n_up"][0])
+        assert np.array_equal(mb["antipar"][i], m1["antipar"][0])
+    if L <= 512:
+        ref = orc.Oracle(L, seeds[0])
+        ref.sweep(6)
+        assert np.array_equal(st[0], ref.export_words())
+    if variant != "fused":
+        batch.set_cycle(B.CYCLE_MIXED)
+        for one in singles:
+            one.set_cycle(B.CYCLE_MIXED)
+        batch.sweep(3)
+        st = batch.get_state().reshape(3, wpr)
+        for i, one in enumerate(singles):
+            one.sweep(3)
+            assert np.array_equal(st[i], one.get_state())
+    batch.free()
+    for one in singles:
+        one.free()
+
+
 # ------------------------------------------------------------------ set_state / structured inputs
 @pytest.mark.parametrize("L,variant", [(64, "generic"), (128, "generic"), (256, "fused"), (256, "generic"),
                                        (64, "resident"), (128, "resident")])
