@@ -317,9 +317,11 @@ def run_ours(args):
     algo_bytes_per_launch = ALGO_BYTES_PER_SITE_UPDATE * N / launches_per_sweep
     achieved = algo_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
     sm_mhz = clocks.get("sm_mhz") or 1965.0
-    # ALU roofline: 13 ALU-pipe (LOP3/SHF) warp-instructions per 32 sites,
-    # 16 lanes/clk/SMSP = 64 thread-ops/clk/SM, 148 SMs, at the SM clock seen during the run
-    alu_ops_per_site = 13.0 / 32.0
+    # Integer issue roofline: the 16-lane integer instructions (LOP3, SHF, IMAD.WIDE)
+    # issue at 0.5 warp-instructions/clk/SMSP = 64 thread-instructions/clk/SM whatever their pipe
+    # (profiles/r1c, r1h); the rule + Philox need 51 + 18 = 69 of them per 128 sites and colour;
+    # 148 SMs at the SM clock seen during the run
+    alu_ops_per_site = 69.0 / 128.0
     alu_bound = 148 * 64 * sm_mhz * 1e6 / alu_ops_per_site / 1e9
     hbm_bound = peak / ALGO_BYTES_PER_SITE_UPDATE
     roofline = {
