@@ -30,9 +30,11 @@
 namespace ising {
 
 #ifndef ISING_F2_STAGES
-#define ISING_F2_STAGES 4
+#define ISING_F2_STAGES 6
 #endif
-constexpr int kF2Stages = ISING_F2_STAGES;     // shared-memory ring depth S; prefetch distance S-1
+// Shared-memory ring depth S; prefetch distance S-1.  The depth itself does not matter (4, 5, 6 time the
+// same); 6 = the unroll depth of the march makes the stage of every step a compile-time constant.
+constexpr int kF2Stages = ISING_F2_STAGES;
 
 // Per-launch Philox constants (host-folded, D5): counter (q, t, colour, 0), key (k0, k1).
 struct SweepConsts {
@@ -131,6 +133,13 @@ __device__ __forceinline__ uint4 xneigh(const uint4 w, const int lane_prev, cons
 // Register windows of one thread: [slot][row]; the slot <-> plane assignment rotates with the
 // step phase PH = k mod 3 (W: slot PH = z-1, PH+1 = z, PH+2 = z+1; B_new: PH = z-2, PH+1 = z-1,
 // PH+2 = z), all indices compile-time after unrolling.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t p;
+    asm volatile("{\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nselp.u32 %0, 1, 0, e;\n}\n" : "=r"(p));
+    return p != 0;
+}
+
 struct F2Win {
     uint4 W[3][2];
     uint4 B[3][2];
@@ -148,17 +157,23 @@ struct F2Ctx {
     int nz;
 };
 
-template <int R4, int PLANE, int PH, int O>
+// U = position of the step in the 6-step unrolled march (k = 6 lap + U).  With a ring of 3 or 6 stages
+// the stage of the step, and with it every shared-memory address, is base + immediate; the mbarrier
+// parity is U/3 (S = 3) or the parity of the lap (S = 6).  The exchange plane index is U & 1.
+template <int R4, int PLANE, int U>
 __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const int z,
-                                        const SweepConsts &keys)
+                                        const uint32_t lap_parity, const SweepConsts &keys)
 {
     constexpr int S = kF2Stages;
+    constexpr int PH = U % 3, O = U & 1;
     constexpr int M = PH % 3, Z = (PH + 1) % 3, P = (PH + 2) % 3;
-    const int s = k % S;
-    mbar_wait(smem_u32(&c.bars[s]), (uint32_t)((k / S) & 1));
+    constexpr bool kStatic = (S == 3 || S == 6);
+    const int s = kStatic ? U % S : k % S;
+    const uint32_t par = S == 3 ? (uint32_t)(U / 3) : S == 6 ? lap_parity : (uint32_t)((k / S) & 1);
+    mbar_wait(smem_u32(&c.bars[s]), par);
     const uint4 *Wnew = c.Wst + s * PLANE;
     const uint4 *Bold = c.Bst + s * PLANE;
-    const uint4 *Wz = c.Wst + ((k + S - 1) % S) * PLANE;          // plane z of W_old
+    const uint4 *Wz = c.Wst + (kStatic ? (U + S - 1) % S : (k + S - 1) % S) * PLANE;   // plane z of W_old
     w.W[P][0] = Wnew[c.si0];
     w.W[P][1] = Wnew[c.si0 + R4];
     const uint4 Bo0 = Bold[c.si0], Bo1 = Bold[c.si0 + R4];
@@ -172,7 +187,7 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
         const uint4 Wx1 = xneigh<1 - O>(w.W[Z][1], c.lane_prev, c.lane_next);
         w.B[P][0] = rule_group(Bo0, rho0, w.W[Z][0], Wx0, Wym, w.W[Z][1], w.W[M][0], w.W[P][0]);
         w.B[P][1] = rule_group(Bo1, rho1, w.W[Z][1], Wx1, w.W[Z][0], Wyp, w.W[M][1], w.W[P][1]);
-        uint4 *nbw = c.nb + (k & 1) * PLANE + c.si0;
+        uint4 *nbw = c.nb + O * PLANE + c.si0;
         nbw[0] = w.B[P][0];
         nbw[R4] = w.B[P][1];
         if (k >= 3 && k < 3 + c.nz) {
@@ -183,7 +198,7 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
     }
     // ---- white update at plane z-1 (colour 1) on the updated black spins ----
     {
-        const uint4 *Bz = c.nb + ((k - 1) & 1) * PLANE;          // B_new[z-1], written last step
+        const uint4 *Bz = c.nb + (1 - O) * PLANE;                // B_new[z-1], written last step
         const uint4 Bym = Bz[c.si_ym], Byp = Bz[c.si_yp];
         const int zw = z == 0 ? (int)(c.qplane / R4) - 1 : z - 1;
         const uint32_t q = (uint32_t)zw * c.qplane + c.qrow;
@@ -275,15 +290,20 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     int pzw = ((zs - 2) % L + L) % L, pzb = ((zs - 3) % L + L) % L, pk = 0;
     const uint4 *pgw = srcW + (size_t)pzw * plane_u4;
     const uint4 *pgb = srcB + (size_t)pzb * plane_u4;
+    // The whole of warp 0 runs the producer: its state is then warp-uniform (uniform registers and
+    // datapath, no per-thread copies of the pointers), and one elected lane issues the copies.
+    const bool prod_warp = __shfl_sync(0xffffffffu, tid >> 5, 0) == 0;
     auto issue_next = [&]() {
         const int s = pk % S;
         const uint32_t bar = smem_u32(&bars[s]);
-        mbar_expect_tx(bar, 2u * (uint32_t)PLANE * 16u);
-        bulk_g2s(smem_u32(Wst + s * PLANE), pgw + (size_t)ybase * R4, bytes1, bar);
-        bulk_g2s(smem_u32(Bst + s * PLANE), pgb + (size_t)ybase * R4, bytes1, bar);
-        if (bytes2) {
-            bulk_g2s(smem_u32(Wst + s * PLANE + n1 * R4), pgw, bytes2, bar);
-            bulk_g2s(smem_u32(Bst + s * PLANE + n1 * R4), pgb, bytes2, bar);
+        if (elect_one()) {
+            mbar_expect_tx(bar, 2u * (uint32_t)PLANE * 16u);
+            bulk_g2s(smem_u32(Wst + s * PLANE), pgw + (size_t)ybase * R4, bytes1, bar);
+            bulk_g2s(smem_u32(Bst + s * PLANE), pgb + (size_t)ybase * R4, bytes1, bar);
+            if (bytes2) {
+                bulk_g2s(smem_u32(Wst + s * PLANE + n1 * R4), pgw, bytes2, bar);
+                bulk_g2s(smem_u32(Bst + s * PLANE + n1 * R4), pgb, bytes2, bar);
+            }
         }
         ++pk;
         pgw += plane_u4;
@@ -291,7 +311,7 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
         if (++pzw == L) { pzw = 0; pgw = srcW; }
         if (++pzb == L) { pzb = 0; pgb = srcB; }
     };
-    if (tid == 0)
+    if (prod_warp)
         for (int k = 0; k < D && k < K; ++k) issue_next();
 
     F2Win w;
@@ -306,22 +326,22 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     if (z < 0) z += L;
     int k = 0;
 
-#define F2_STEP(PH, O)                                                        \
+#define F2_STEP(U)                                                            \
     {                                                                         \
         if (k >= K) break;                                                    \
-        f2_step<R4, PLANE, PH, O>(w, c, k, z, keys);                          \
+        f2_step<R4, PLANE, U>(w, c, k, z, lap_parity, keys);                  \
         __syncthreads();                                                      \
-        if (tid == 0 && pk < K) issue_next();                                 \
+        if (prod_warp && pk < K) issue_next();                                \
         ++k;                                                                  \
         z = (z + 1 == L) ? 0 : z + 1;                                         \
     }
-    for (;;) {
-        F2_STEP(0, 0)
-        F2_STEP(1, 1)
-        F2_STEP(2, 0)
-        F2_STEP(0, 1)
-        F2_STEP(1, 0)
-        F2_STEP(2, 1)
+    for (uint32_t lap_parity = 0;; lap_parity ^= 1u) {
+        F2_STEP(0)
+        F2_STEP(1)
+        F2_STEP(2)
+        F2_STEP(3)
+        F2_STEP(4)
+        F2_STEP(5)
     }
 #undef F2_STEP
 }
