@@ -161,8 +161,9 @@ struct F2Ctx {
 // the stage of the step, and with it every shared-memory address, is base + immediate; the mbarrier
 // parity is U/3 (S = 3) or the parity of the lap (S = 6).  The exchange plane index is U & 1.
 template <int R4, int PLANE, int U>
-__device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const int z,
-                                        const uint32_t lap_parity, const SweepConsts &keys)
+__device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const uint32_t qb,
+                                        const uint32_t qw, const uint32_t lap_parity,
+                                        const SweepConsts &keys)
 {
     constexpr int S = kF2Stages;
     constexpr int PH = U % 3, O = U & 1;
@@ -180,7 +181,7 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
     // ---- black update at plane z (colour 0); even row: o = O, odd row: o = 1-O ----
     {
         const uint4 Wym = Wz[c.si_ym], Wyp = Wz[c.si_yp];
-        const uint32_t q = (uint32_t)z * c.qplane + c.qrow;
+        const uint32_t q = qb;                                    // group of (row 2p, x4) in plane z
         const uint4 rho0 = philox_folded<0>(q, keys);
         const uint4 rho1 = philox_folded<0>(q + R4, keys);
         const uint4 Wx0 = xneigh<O>(w.W[Z][0], c.lane_prev, c.lane_next);
@@ -191,7 +192,7 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
         nbw[0] = w.B[P][0];
         nbw[R4] = w.B[P][1];
         if (k >= 3 && k < 3 + c.nz) {
-            uint4 *d = c.dstB + (size_t)((uint32_t)z * c.qplane + c.qrow);
+            uint4 *d = c.dstB + (size_t)q;
             if (c.ok0) d[0] = w.B[P][0];
             if (c.ok1) d[R4] = w.B[P][1];
         }
@@ -200,8 +201,7 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
     {
         const uint4 *Bz = c.nb + (1 - O) * PLANE;                // B_new[z-1], written last step
         const uint4 Bym = Bz[c.si_ym], Byp = Bz[c.si_yp];
-        const int zw = z == 0 ? (int)(c.qplane / R4) - 1 : z - 1;
-        const uint32_t q = (uint32_t)zw * c.qplane + c.qrow;
+        const uint32_t q = qw;                                    // the same group in plane z-1
         const uint4 rho0 = philox_folded<1>(q, keys);
         const uint4 rho1 = philox_folded<1>(q + R4, keys);
         const uint4 Bx0 = xneigh<O>(w.B[Z][0], c.lane_prev, c.lane_next);
@@ -263,6 +263,8 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     const uint4 *srcB = src + (first ? G : 0), *srcW = src + (first ? 0 : G);
     c.dstB = dst + (first ? G : 0);
     c.dstW = dst + (first ? 0 : G);
+    // keep the two store bases as plain 64-bit values (address = base + 16 q: one LEA pair per store)
+    asm volatile("" : "+l"(c.dstB), "+l"(c.dstW));
     c.si0 = ry * R4 + x4;
     c.si_ym = ry > 0 ? c.si0 - R4 : c.si0;
     c.si_yp = ry + 2 < TY ? c.si0 + 2 * R4 : c.si0;
@@ -325,15 +327,21 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     int z = zs - 3;                        // plane of the black update (even)
     if (z < 0) z += L;
     int k = 0;
+    // Philox / store group index of this thread's even row in the black plane z (qb) and in the white
+    // plane z-1 (qw = the previous step's qb), kept incrementally
+    uint32_t qb = (uint32_t)z * c.qplane + c.qrow;
+    uint32_t qw = (uint32_t)(z == 0 ? L - 1 : z - 1) * c.qplane + c.qrow;
 
 #define F2_STEP(U)                                                            \
     {                                                                         \
         if (k >= K) break;                                                    \
-        f2_step<R4, PLANE, U>(w, c, k, z, lap_parity, keys);                  \
+        f2_step<R4, PLANE, U>(w, c, k, qb, qw, lap_parity, keys);             \
         __syncthreads();                                                      \
         if (prod_warp && pk < K) issue_next();                                \
         ++k;                                                                  \
         z = (z + 1 == L) ? 0 : z + 1;                                         \
+        qw = qb;                                                              \
+        qb = z == 0 ? c.qrow : qb + c.qplane;                                 \
     }
     for (uint32_t lap_parity = 0;; lap_parity ^= 1u) {
         F2_STEP(0)
