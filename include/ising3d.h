@@ -211,6 +211,16 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream);
 int ising3d_set_variant(ising3d_t *h, int variant);
 
 /*
+ * Thread-block cluster size of the resident kernel (L in {64,128,256}): the lattice is split
+ * into `cs` z slabs, one CTA (= one SM) each, halo planes exchanged through distributed shared
+ * memory after every half-sweep.  cs = 0 restores the automatic choice (the
+ * smallest cluster whose slab fits shared memory, grown while all replicas stay co-resident).
+ * The result does not depend on cs.  EINVAL unless cs is a power of two <= 16 with L/cs >= 2
+ * whose slab fits 200 KB of shared memory and that the device can schedule, or for other L.
+ */
+int ising3d_set_cluster_size(ising3d_t *h, int cs);
+
+/*
  * Run n_sweeps checkerboard sweeps (eq. (6)).
  * Asynchronous on the handle's stream; no host synchronisation inside.
  * The sweep counter advances by n_sweeps; EINVAL if it would pass 2^32-1.

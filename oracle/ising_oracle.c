@@ -35,8 +35,10 @@
  *   orc_first_colour / orc_sweep_mixed : Neel state closed form (the first colour
  *                         decides the sign of the ordered state), bit statistics,
  *                         big-integer Python Philox
- *   orc_menger_solid / orc_init_menger : solid counts 20^k, the k = 1 cross written
- *                         out, self-similarity, tile-sign statistics, k = 0 iid
+ *   orc_menger_solid / orc_init_menger / orc_menger_site : solid counts 20^k, the k = 1 cross
+ *                         written out, self-similarity, tile-sign statistics, k = 0 iid; the
+ *                         single-site form equals the array form site by site and the big-integer
+ *                         Python Philox on tiles beyond 2^32
  *   orc_corr_direct / orc_radial_bin / orc_radial_sums : P(0) = N, sum_d P(d) = M^2,
  *                         P along the axes = N - 2 A_mu(r) (orc_measure), slab closed form,
  *                         shell counts against a set-based Python count, bins vs exact
@@ -419,6 +421,25 @@ void orc_init_menger(orc_t *o, int k)
                 o->s[orc_idx(o, x, y, z)] = (int8_t)(solid ? sign : -sign);
             }
     o->sweep = 0;
+}
+
+/* The same start for one site (D11 written out for (x,y,z) alone): for */
+/* sampled-site parity at sizes where the array version is too slow     */
+/* (L = 2048, k = 0: the tile index passes 2^32).  Pinned against       */
+/* orc_init_menger site by site on small L and against the big-integer  */
+/* Python Philox on hand-indexed tiles of L = 2048 (test_oracle_next).  */
+int orc_menger_site(uint64_t seed, int L, int k, int x, int y, int z)
+{
+    int size = 1;
+    for (int i = 0; i < k; ++i) size *= 3;
+    const uint64_t nT = (uint64_t)((L + size - 1) / size);
+    const uint64_t T = ((uint64_t)(z / size) * nT + (uint64_t)(y / size)) * nT + (uint64_t)(x / size);
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t ctr[4] = { (uint32_t)(T >> 7), (uint32_t)k, 0u, 3u };
+    uint32_t out[4];
+    orc_philox4x32_10(ctr, key, out);
+    const int sign = ((out[(T >> 5) & 3] >> (T & 31)) & 1u) ? 1 : -1;
+    return orc_menger_solid(x % size, y % size, z % size, k) ? sign : -sign;
 }
 
 /* ------------------------------------------------------------------ */

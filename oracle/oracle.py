@@ -96,6 +96,8 @@ def lib():
         l.orc_menger_solid.restype = C.c_int
         l.orc_init_menger.argtypes = [C.c_void_p, C.c_int]
         l.orc_init_menger.restype = None
+        l.orc_menger_site.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+        l.orc_menger_site.restype = C.c_int
         i64p = C.POINTER(C.c_int64)
         l.orc_radial_bin.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int]
         l.orc_radial_bin.restype = C.c_int
@@ -164,6 +166,11 @@ def first_colour(seed: int, t: int) -> int:
 def menger_solid(u: int, v: int, w: int, k: int) -> int:
     """1 iff (u,v,w) in [0,3^k)^3 belongs to the k-th iteration Menger sponge."""
     return int(lib().orc_menger_solid(int(u), int(v), int(w), int(k)))
+
+
+def menger_site(seed: int, L: int, k: int, x: int, y: int, z: int) -> int:
+    """Spin (+-1) of site (x,y,z) in the Menger start of iteration k (D11), one site at a time."""
+    return int(lib().orc_menger_site(int(seed), int(L), int(k), int(x), int(y), int(z)))
 
 
 def radial_bin(L: int, dx: int, dy: int, dz: int) -> int:

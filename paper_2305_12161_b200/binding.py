@@ -28,7 +28,8 @@ EXPORTED = [
     "ising3d_measure_variant_name",
     "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
-    "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size", "ising3d_sync",
+    "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size",
+    "ising3d_set_cluster_size", "ising3d_sync",
     "ising3d_free", "ising3d_last_error",
 ]
 
@@ -95,6 +96,7 @@ def load():
         "ising3d_launch_count": (u64, [vp]),
         "ising3d_variant_name": (C.c_char_p, [vp]),
         "ising3d_cluster_size": (C.c_int, [vp]),
+        "ising3d_set_cluster_size": (C.c_int, [vp, C.c_int]),
         "ising3d_sync": (C.c_int, [vp]),
         "ising3d_free": (None, [vp]),
         "ising3d_last_error": (C.c_char_p, []),
@@ -181,6 +183,9 @@ class Ising3D:
 
     def set_variant(self, variant: int):
         _check(self._l.ising3d_set_variant(self._h, variant))
+
+    def set_cluster_size(self, cs: int):
+        _check(self._l.ising3d_set_cluster_size(self._h, int(cs)))
 
     def set_measure_variant(self, variant: int):
         _check(self._l.ising3d_set_measure_variant(self._h, variant))

@@ -28,9 +28,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             and os.path.getmtime(LIB) >= max(os.path.getmtime(s) for s in srcs)):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
-    # ISING3D_NVCC_EXTRA: extra nvcc arguments (e.g. "-DISING_F2_STAGES=5") for kernel experiments
-    extra = os.environ.get("ISING3D_NVCC_EXTRA", "").split()
-    cmd = ["nvcc"] + NVCC_FLAGS + extra + ["-o", tmp, os.path.join(CSRC, "ising3d.cu")]
+    cmd = ["nvcc"] + NVCC_FLAGS + ["-o", tmp, os.path.join(CSRC, "ising3d.cu")]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
@@ -39,24 +37,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
         sys.stderr.write(res.stdout + res.stderr)
     os.replace(tmp, LIB)
     return LIB
-
-
-MICROBENCHMARKS = ["pipe_rates.cu", "sweep_ceiling.cu"]     # standalone programs behind profiles/r1c, r1h
-
-
-def build_microbenchmarks(out_dir: str) -> list:
-    """Compile the standalone microbenchmarks (not part of the library) for sm_100a into out_dir."""
-    outs = []
-    for src in MICROBENCHMARKS:
-        exe = os.path.join(out_dir, os.path.splitext(src)[0])
-        cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-               "-o", exe, os.path.join(_HERE, src)]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if res.returncode != 0:
-            sys.stderr.write(res.stdout + res.stderr)
-            raise RuntimeError("nvcc failed building " + src)
-        outs.append(exe)
-    return outs
 
 
 if __name__ == "__main__":

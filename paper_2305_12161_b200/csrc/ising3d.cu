@@ -76,6 +76,10 @@ struct ising3d {
     int sm_count = 148;
     mutable ising::ResidentPlan res_plan = {0, 0};
     mutable bool res_planned = false;
+    // launch shapes and per-device function attributes, set up at the handle's first use of a
+    // kernel (nothing process-wide: distinct handles are independent, include/ising3d.h)
+    ising::FusedPlan plan_f1, plan_f2, plan_f3;
+    bool attr_gram = false, attr_autocorr = false;
 
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
@@ -92,12 +96,6 @@ struct ising3d {
         if (!ising::resident_supported(L)) return false;
         if (!res_planned) {
             res_plan = ising::resident_plan(L, n_rep, sm_count);
-            if (const char *e = getenv("ISING3D_RESIDENT_CS")) {     // experiments only
-                const int cs = atoi(e);
-                if (cs >= 1 && cs <= 16 && L % cs == 0 && L / cs >= 2 &&
-                    ising::resident_smem_bytes(L, cs) <= 200 * 1024)
-                    res_plan = ising::ResidentPlan{cs, ising::resident_smem_bytes(L, cs)};
-            }
             res_planned = true;
         }
         return res_plan.cs > 0;
@@ -290,12 +288,21 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
 {
     const size_t wpr = h->words_per_replica();
     uint64_t i = 0;
+    {
+        cudaError_t e = cudaSuccess;
+        if (gen2 && !h->plan_f2.ready) e = ising::plan_fused2(h->plan_f2, h->L, h->sm_count);
+        if (e == cudaSuccess && !gen2 && !h->plan_f1.ready) e = ising::plan_fused(h->plan_f1, h->L, h->sm_count);
+        if (e == cudaSuccess && gen2 && h->use_fused3() && !h->plan_f3.ready)
+            e = ising::plan_fused3(h->plan_f3, h->L, h->sm_count);
+        if (e != cudaSuccess)
+            return fail(ISING3D_ECUDA, std::string("fused sweep plan: ") + cudaGetErrorString(e));
+    }
     // pairs of sweeps with the intermediate state on chip (01 cycle); an odd last sweep below
     for (; gen2 && h->use_fused3() && i + 2 <= n; i += 2) {
         for (int rep = 0; rep < h->n_rep; ++rep) {
             cudaError_t e = ising::launch_fused3_sweep2(
                 h->state[h->cur] + rep * wpr, h->state[1 - h->cur] + rep * wpr, h->L,
-                (uint32_t)(h->sweep + i), h->seeds[rep], h->sm_count, h->stream);
+                (uint32_t)(h->sweep + i), h->seeds[rep], h->plan_f3, h->stream);
             if (e != cudaSuccess)
                 return fail(ISING3D_ECUDA, std::string("fused3 sweep launch: ") + cudaGetErrorString(e));
         }
@@ -311,9 +318,9 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
             // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
             const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
             cudaError_t e =
-                gen2 ? ising::launch_fused2_sweep(src, dst, h->L, t, seed, first, h->sm_count, h->stream)
+                gen2 ? ising::launch_fused2_sweep(src, dst, h->L, t, seed, first, h->plan_f2, h->stream)
                      : ising::launch_fused_sweep(src, dst, h->L, t, ising::make_philox_keys(seed),
-                                                 h->sm_count, h->stream);
+                                                 h->plan_f1, h->stream);
             if (e != cudaSuccess)
                 return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
         }
@@ -402,20 +409,16 @@ int fft_setup(ising3d *h)
 int measure_gram(ising3d *h)
 {
     const int L = h->L, nr = L / 2 + 1, cpr = h->counts_per_replica();
-    static unsigned long long attr_set = 0;     // bit per device: function attributes are per device
-    int dev = 0;
-    CUDA_TRY(cudaGetDevice(&dev));
-    const unsigned long long dev_bit = 1ull << (dev & 63);
     const ising::GramPlan plan = ising::make_gram_plan(L, h->sm_count);
     const size_t smem = ising::gram_smem_bytes(L, plan);
     const int NWB = 4;                         // row words per block of the x gather
     const size_t smem_x = ((size_t)64 * NWB * (L / 32 + 1) + (size_t)2 * 256 * (NWB + 1)) * 4;
-    if (!(attr_set & dev_bit)) {
+    if (!h->attr_gram) {       // per device, idempotent; once per handle
         CUDA_TRY(cudaFuncSetAttribute(ising::gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       210 * 1024));
         CUDA_TRY(cudaFuncSetAttribute(ising::gather_lines_x_kernel,
                                       cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-        attr_set |= dev_bit;
+        h->attr_gram = true;
     }
     CUDA_TRY(cudaMemsetAsync(h->d_gsum, 0, (size_t)h->n_rep * 3 * nr * 8, h->stream));
     CUDA_TRY(cudaMemsetAsync(h->d_queue, 0, (size_t)h->n_rep * 3 * 4, h->stream));
@@ -580,6 +583,28 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     return ISING3D_OK;
 }
 
+int ising3d_set_cluster_size(ising3d_t *h, int cs)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (!ising::resident_supported(h->L))
+        return fail(ISING3D_EINVAL, "the resident kernel needs L in {64,128,256}");
+    if (cs == 0) {                               // back to the automatic choice
+        h->res_planned = false;
+        return ISING3D_OK;
+    }
+    if (cs < 1 || cs > 16 || (cs & (cs - 1)) || h->L / cs < 2 ||
+        ising::resident_smem_bytes(h->L, cs) > 200 * 1024)
+        return fail(ISING3D_EINVAL, "cluster size must be a power of two <= 16 whose z slab fits shared memory");
+    int clusters = 0;
+    if (ising::resident_try_size(h->L, cs, h->n_rep, &clusters) != cudaSuccess || clusters < 1) {
+        cudaGetLastError();
+        return fail(ISING3D_EINVAL, "this device cannot co-schedule a cluster of that size");
+    }
+    h->res_plan = ising::ResidentPlan{cs, ising::resident_smem_bytes(h->L, cs)};
+    h->res_planned = true;
+    return ISING3D_OK;
+}
+
 int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
@@ -621,11 +646,7 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
         const int C = ising::autocorr_tile_sequences(L);
         const int n_tiles = (L * L / 32) / C;
         const size_t smem = ising::autocorr_smem_bytes(L, C);
-        static unsigned long long attr_set = 0;     // bit per device
-        int dev = 0;
-        CUDA_TRY(cudaGetDevice(&dev));
-        const unsigned long long dev_bit = 1ull << (dev & 63);
-        if (!(attr_set & dev_bit)) {
+        if (!h->attr_autocorr) {                    // per device, idempotent; once per handle
             const int max_smem = (int)ising::autocorr_smem_bytes(4096, 8) + 4096;
             CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<0>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
@@ -633,7 +654,7 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
             CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<2>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-            attr_set |= dev_bit;
+            h->attr_autocorr = true;
         }
         int gx = std::max(1, (h->sm_count + h->n_rep - 1) / h->n_rep);
         gx = std::min(gx, n_tiles);

@@ -241,42 +241,45 @@ inline bool fused_supported(int L)
     return L == 256 || L == 512 || L == 1024 || L == 2048 || L == 4096;
 }
 
+// Launch shape of a fused sweep kernel for one (L, device): computed once per handle at its first
+// sweep and kept in the handle (no process-wide state: distinct handles are independent).
 struct FusedPlan {
-    int nty, RPT, nzc;
-    size_t smem;
+    int nty = 0, RPT = 0, nzc = 0;
+    bool ready = false;
 };
 
 template <int R4, int NT>
-inline cudaError_t launch_fused_t(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
-                                  const PhiloxKeys &keys, int sm_count, cudaStream_t stream)
+inline cudaError_t plan_fused_t(FusedPlan &plan, int L, int sm_count)
 {
     constexpr int TY = NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kFusedStages + 2) + kFusedStages * 8;
-    static FusedPlan plan = {0, 0, 0, 0};
-    static int plan_L = 0, plan_sms = 0, plan_dev = -1;   // attributes are per device
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
-        cudaError_t e = cudaFuncSetAttribute(fused_sweep_kernel<R4, NT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        int occ = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_sweep_kernel<R4, NT>, NT, smem);
-        if (e != cudaSuccess) return e;
-        if (occ < 1) occ = 1;
-        const int tyo = TY - 4;
-        plan.nty = (L + tyo - 1) / tyo;
-        plan.RPT = (L + plan.nty - 1) / plan.nty;
-        int nzc = (sm_count * occ) / plan.nty;
-        if (nzc < 1) nzc = 1;
-        if (nzc > L / 8) nzc = L / 8;
-        plan.nzc = nzc;
-        plan.smem = smem;
-        plan_L = L;
-        plan_sms = sm_count;
-        plan_dev = dev;
-    }
+    // per device and idempotent; the CUDA runtime serialises concurrent callers
+    cudaError_t e = cudaFuncSetAttribute(fused_sweep_kernel<R4, NT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused_sweep_kernel<R4, NT>, NT, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    const int tyo = TY - 4;
+    plan.nty = (L + tyo - 1) / tyo;
+    plan.RPT = (L + plan.nty - 1) / plan.nty;
+    int nzc = (sm_count * occ) / plan.nty;
+    if (nzc < 1) nzc = 1;
+    if (nzc > L / 8) nzc = L / 8;
+    plan.nzc = nzc;
+    plan.ready = true;
+    return cudaSuccess;
+}
+
+template <int R4, int NT>
+inline cudaError_t launch_fused_t(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
+                                  const PhiloxKeys &keys, const FusedPlan &plan, cudaStream_t stream)
+{
+    constexpr int TY = NT / R4;
+    constexpr int PLANE = TY * R4;
+    constexpr size_t smem = (size_t)PLANE * 16 * (2 * kFusedStages + 2) + kFusedStages * 8;
     dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
     fused_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(
         reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, t, plan.RPT,
@@ -284,15 +287,27 @@ inline cudaError_t launch_fused_t(const uint32_t *src, uint32_t *dst, int L, uin
     return cudaGetLastError();
 }
 
-inline cudaError_t launch_fused_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
-                                      const PhiloxKeys &keys, int sm_count, cudaStream_t stream)
+inline cudaError_t plan_fused(FusedPlan &plan, int L, int sm_count)
 {
     switch (L) {
-        case 256:  return launch_fused_t<1, 256>(src, dst, L, t, keys, sm_count, stream);
-        case 512:  return launch_fused_t<2, 256>(src, dst, L, t, keys, sm_count, stream);
-        case 1024: return launch_fused_t<4, 256>(src, dst, L, t, keys, sm_count, stream);
-        case 2048: return launch_fused_t<8, 256>(src, dst, L, t, keys, sm_count, stream);
-        case 4096: return launch_fused_t<16, 512>(src, dst, L, t, keys, sm_count, stream);
+        case 256:  return plan_fused_t<1, 256>(plan, L, sm_count);
+        case 512:  return plan_fused_t<2, 256>(plan, L, sm_count);
+        case 1024: return plan_fused_t<4, 256>(plan, L, sm_count);
+        case 2048: return plan_fused_t<8, 256>(plan, L, sm_count);
+        case 4096: return plan_fused_t<16, 512>(plan, L, sm_count);
+        default:   return cudaErrorInvalidValue;
+    }
+}
+
+inline cudaError_t launch_fused_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
+                                      const PhiloxKeys &keys, const FusedPlan &plan, cudaStream_t stream)
+{
+    switch (L) {
+        case 256:  return launch_fused_t<1, 256>(src, dst, L, t, keys, plan, stream);
+        case 512:  return launch_fused_t<2, 256>(src, dst, L, t, keys, plan, stream);
+        case 1024: return launch_fused_t<4, 256>(src, dst, L, t, keys, plan, stream);
+        case 2048: return launch_fused_t<8, 256>(src, dst, L, t, keys, plan, stream);
+        case 4096: return launch_fused_t<16, 512>(src, dst, L, t, keys, plan, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

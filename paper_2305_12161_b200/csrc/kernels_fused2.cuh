@@ -29,12 +29,9 @@
 
 namespace ising {
 
-#ifndef ISING_F2_STAGES
-#define ISING_F2_STAGES 6
-#endif
 // Shared-memory ring depth S; prefetch distance S-1.  The depth itself does not matter (4, 5, 6 time the
 // same); 6 = the unroll depth of the march makes the stage of every step a compile-time constant.
-constexpr int kF2Stages = ISING_F2_STAGES;
+constexpr int kF2Stages = 6;
 
 // Per-launch Philox constants (host-folded, D5): counter (q, t, colour, 0), key (k0, k1).
 struct SweepConsts {
@@ -360,51 +357,68 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
 inline bool fused2_supported(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096; }
 
 template <int R4, int NT>
-inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first,
-                                   const SweepConsts &keys, int sm_count, cudaStream_t stream)
+inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
 {
     constexpr int TY = 2 * NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
-    // function attributes are per device: the plan is keyed on the current device as well
-    static int plan_L = 0, plan_sms = 0, plan_dev = -1, nty = 0, RPT = 0, nzc = 0;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
-        cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        int occ = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT>, NT, smem);
-        if (e != cudaSuccess) return e;
-        if (occ < 1) occ = 1;
-        const int tyo = TY - 4;                        // stored rows per tile (even)
-        nty = (L + tyo - 1) / tyo;
-        RPT = (L + nty - 1) / nty;
-        RPT += RPT & 1;                                // even, so that ybase is even
-        nty = (L + RPT - 1) / RPT;
-        nzc = (sm_count * occ) / nty;
-        if (nzc < 1) nzc = 1;
-        if (nzc > L / 8) nzc = L / 8;
-        plan_L = L;
-        plan_sms = sm_count;
-        plan_dev = dev;
-    }
-    dim3 grid((unsigned)nty, (unsigned)nzc);
+    cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT>, NT, smem);
+    if (e != cudaSuccess) return e;
+    if (occ < 1) occ = 1;
+    const int tyo = TY - 4;                        // stored rows per tile (even)
+    int nty = (L + tyo - 1) / tyo;
+    int RPT = (L + nty - 1) / nty;
+    RPT += RPT & 1;                                // even, so that ybase is even
+    nty = (L + RPT - 1) / RPT;
+    int nzc = (sm_count * occ) / nty;
+    if (nzc < 1) nzc = 1;
+    if (nzc > L / 8) nzc = L / 8;
+    plan.nty = nty;
+    plan.RPT = RPT;
+    plan.nzc = nzc;
+    plan.ready = true;
+    return cudaSuccess;
+}
+
+template <int R4, int NT>
+inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first,
+                                   const SweepConsts &keys, const FusedPlan &plan, cudaStream_t stream)
+{
+    constexpr int TY = 2 * NT / R4;
+    constexpr int PLANE = TY * R4;
+    constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
+    dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
     fused2_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(
-        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, RPT, nzc, first, keys);
+        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
+        first, keys);
     return cudaGetLastError();
 }
 
+inline cudaError_t plan_fused2(FusedPlan &plan, int L, int sm_count)
+{
+    switch (L) {
+        case 512:  return plan_fused2_t<2, 128>(plan, L, sm_count);
+        case 1024: return plan_fused2_t<4, 256>(plan, L, sm_count);
+        case 2048: return plan_fused2_t<8, 256>(plan, L, sm_count);
+        case 4096: return plan_fused2_t<16, 256>(plan, L, sm_count);
+        default:   return cudaErrorInvalidValue;
+    }
+}
+
 inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
-                                       uint64_t seed, int first, int sm_count, cudaStream_t stream)
+                                       uint64_t seed, int first, const FusedPlan &plan,
+                                       cudaStream_t stream)
 {
     const SweepConsts keys = make_sweep_consts(seed, t, first);
     switch (L) {
-        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, keys, sm_count, stream);
-        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, keys, sm_count, stream);
-        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, keys, sm_count, stream);
-        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, keys, sm_count, stream);
+        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, keys, plan, stream);
+        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, keys, plan, stream);
+        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, keys, plan, stream);
+        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, keys, plan, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

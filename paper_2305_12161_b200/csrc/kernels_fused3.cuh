@@ -29,14 +29,8 @@
 
 namespace ising {
 
-#ifndef ISING_F3_MID
-#define ISING_F3_MID 8
-#endif
-#ifndef ISING_F3_STAGES
-#define ISING_F3_STAGES 3
-#endif
-constexpr int kF3Mid = ISING_F3_MID;        // SM: planes of B1 / W1 kept in shared memory
-constexpr int kF3Stages = ISING_F3_STAGES;  // S: bulk-copy ring depth of level 1
+constexpr int kF3Mid = 8;                   // SM: planes of B1 / W1 kept in shared memory
+constexpr int kF3Stages = 3;                // S: bulk-copy ring depth of level 1
 constexpr int kF3Dz = 2;                    // DZ
 
 __device__ __forceinline__ void named_bar_sync(const int id, const int count)
@@ -326,47 +320,62 @@ fused3_sweep2_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, con
 inline bool fused3_supported(int L) { return L == 1024 || L == 2048; }
 
 template <int R4, int NT>
-inline cudaError_t launch_fused3_t(const uint32_t *src, uint32_t *dst, int L, const SweepConsts &k1,
-                                   const SweepConsts &k2, int sm_count, cudaStream_t stream)
+inline cudaError_t plan_fused3_t(FusedPlan &plan, int L, int sm_count)
 {
     constexpr int TY = 2 * NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem =
         (size_t)PLANE * 16 * (2 * kF3Stages + 2 * kF3Mid + 2) + kF3Stages * 8 + 16;
-    // function attributes are per device: the plan is keyed on the current device as well
-    static int plan_L = 0, plan_sms = 0, plan_dev = -1, nty = 0, RPT = 0, nzc = 0;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (plan_L != L || plan_sms != sm_count || plan_dev != dev) {
-        cudaError_t e = cudaFuncSetAttribute(fused3_sweep2_kernel<R4, NT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        const int tyo = TY - 8;                        // stored rows per tile (even)
-        nty = (L + tyo - 1) / tyo;
-        RPT = (L + nty - 1) / nty;
-        RPT += RPT & 1;
-        nty = (L + RPT - 1) / RPT;
-        nzc = sm_count / nty;                          // one CTA per SM
-        if (nzc < 1) nzc = 1;
-        if (nzc > L / 16) nzc = L / 16;
-        plan_L = L;
-        plan_sms = sm_count;
-        plan_dev = dev;
-    }
-    dim3 grid((unsigned)nty, (unsigned)nzc);
+    cudaError_t e = cudaFuncSetAttribute(fused3_sweep2_kernel<R4, NT>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int tyo = TY - 8;                        // stored rows per tile (even)
+    int nty = (L + tyo - 1) / tyo;
+    int RPT = (L + nty - 1) / nty;
+    RPT += RPT & 1;
+    nty = (L + RPT - 1) / RPT;
+    int nzc = sm_count / nty;                      // one CTA per SM
+    if (nzc < 1) nzc = 1;
+    if (nzc > L / 16) nzc = L / 16;
+    plan.nty = nty;
+    plan.RPT = RPT;
+    plan.nzc = nzc;
+    plan.ready = true;
+    return cudaSuccess;
+}
+
+template <int R4, int NT>
+inline cudaError_t launch_fused3_t(const uint32_t *src, uint32_t *dst, int L, const SweepConsts &k1,
+                                   const SweepConsts &k2, const FusedPlan &plan, cudaStream_t stream)
+{
+    constexpr int TY = 2 * NT / R4;
+    constexpr int PLANE = TY * R4;
+    constexpr size_t smem =
+        (size_t)PLANE * 16 * (2 * kF3Stages + 2 * kF3Mid + 2) + kF3Stages * 8 + 16;
+    dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
     fused3_sweep2_kernel<R4, NT><<<grid, 2 * NT, smem, stream>>>(
-        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, RPT, nzc, k1, k2);
+        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
+        k1, k2);
     return cudaGetLastError();
+}
+
+inline cudaError_t plan_fused3(FusedPlan &plan, int L, int sm_count)
+{
+    switch (L) {
+        case 1024: return plan_fused3_t<4, 256>(plan, L, sm_count);
+        case 2048: return plan_fused3_t<8, 256>(plan, L, sm_count);
+        default:   return cudaErrorInvalidValue;
+    }
 }
 
 // sweeps t and t+1 (cycle 01) of the state `src` into `dst`
 inline cudaError_t launch_fused3_sweep2(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
-                                        uint64_t seed, int sm_count, cudaStream_t stream)
+                                        uint64_t seed, const FusedPlan &plan, cudaStream_t stream)
 {
     const SweepConsts k1 = make_sweep_consts(seed, t, 0), k2 = make_sweep_consts(seed, t + 1, 0);
     switch (L) {
-        case 1024: return launch_fused3_t<4, 256>(src, dst, L, k1, k2, sm_count, stream);
-        case 2048: return launch_fused3_t<8, 256>(src, dst, L, k1, k2, sm_count, stream);
+        case 1024: return launch_fused3_t<4, 256>(src, dst, L, k1, k2, plan, stream);
+        case 2048: return launch_fused3_t<8, 256>(src, dst, L, k1, k2, plan, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

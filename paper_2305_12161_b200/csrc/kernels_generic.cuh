@@ -79,9 +79,10 @@ init_menger_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ se
             if (ones >= 2) solid = false;
             a /= 3; b /= 3; d /= 3;
         }
-        const uint32_t T = (uint32_t)((Z * nT + Y) * nT + X);
-        if ((T >> 7) != cached_group) {
-            cached_group = T >> 7;
+        // 64-bit tile index: nT^3 passes 2^32 from L = 1664 at k = 0 (the counter word is T >> 7)
+        const uint64_t T = ((uint64_t)Z * (uint64_t)nT + (uint64_t)Y) * (uint64_t)nT + (uint64_t)X;
+        if ((uint32_t)(T >> 7) != cached_group) {
+            cached_group = (uint32_t)(T >> 7);
             rnd = philox4x32_10(cached_group, (uint32_t)k, 0u, kTagMenger, (uint32_t)seed,
                                 (uint32_t)(seed >> 32));
         }

@@ -224,6 +224,10 @@ inline GramPlan make_gram_plan(int L, int sm_count)
     p.n_stages = kGramMaxStages;
     const int tiles = (L / 128) * p.n_groups;
     p.n_slices = (sm_count * 12 + tiles - 1) / tiles;
+    // the s32 accumulators hold 128 * G, G <= lines per slice: keep 128 * K_slice < 2^31 on any device
+    const long long kmax = (1ll << 31) / 128 - 1;
+    const int min_slices = (int)(((long long)L * L + kmax - 1) / kmax);
+    if (p.n_slices < min_slices) p.n_slices = min_slices;
     p.n_tasks = p.n_slices * tiles;
     return p;
 }
@@ -283,6 +287,12 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
     int rs = 0;                                        // ring position: stage rs, wrap parity rp
     uint32_t rp = 0;
     int n_done = 0;                                    // tasks finished by this CTA
+    // hist[] is 32-bit: a task adds at most 128 pairs * 128 lines per chunk to one r.  `hist_bound`
+    // (CTA-uniform) bounds what one entry may hold; the histogram is flushed to the 64-bit global
+    // sums before another task could pass 2^32, whatever the SM count or the queue balance.
+    unsigned long long hist_bound = 0;
+    const unsigned long long task_max =
+        128ull * 128ull * (unsigned long long)((n_chunks + plan.n_slices - 1) / plan.n_slices + 1);
     for (int task = task_s[0]; task < plan.n_tasks; ++n_done) {
         // decode: slice-major so that concurrently running CTAs read the same K range (L2 reuse)
         const int slice = task / tiles_per_slice, tl = task - slice * tiles_per_slice;
@@ -420,6 +430,15 @@ gram_kernel(const uint32_t *__restrict__ xw, unsigned long long *__restrict__ gs
         if (tid == 0) task_s[(n_done + 1) & 1] = (int)atomicAdd(queue, 1u);
         __syncthreads();
         task = task_s[(n_done + 1) & 1];
+        hist_bound += task_max;
+        if (hist_bound + task_max > 0xFFFFFFFFull) {
+            for (int r = 1 + tid; r <= half; r += kGramThreads) {
+                if (hist[r]) atomicAdd(&gsum[r], (unsigned long long)hist[r]);
+                hist[r] = 0;
+            }
+            hist_bound = 0;
+            __syncthreads();
+        }
     }
 
     asm volatile("tcgen05.fence::before_thread_sync;");

@@ -175,6 +175,10 @@ autocorr_kernel(const uint32_t *__restrict__ state, unsigned long long *__restri
     const int nr = L / 2 + 1;
 
     for (int r = tid; r < nr; r += kAcThreads) cnt[r] = 0;
+    // cnt[] is 32-bit: one tile adds at most 32 * C * L (= 2^20 for full tiles) to an entry, so it is
+    // flushed to the 64-bit global counters every `flush_every` tiles, whatever the grid size
+    const int flush_every = (int)(0xFFFFFFFFull / (32ull * (unsigned long long)C * (unsigned long long)L));
+    int since_flush = 0;
 
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         __syncthreads();                     // previous tile fully consumed, cnt zeroed
@@ -266,6 +270,16 @@ autocorr_kernel(const uint32_t *__restrict__ state, unsigned long long *__restri
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             if (lane == 0) atomicAdd(&cnt[half], acc);
+        }
+        if (++since_flush >= flush_every) {
+            __syncthreads();
+            for (int r = 1 + tid; r < nr; r += kAcThreads) {
+                if (cnt[r])
+                    atomicAdd(&counts[(size_t)rep * counts_per_replica + 1 + AX * nr + r],
+                              (unsigned long long)cnt[r]);
+                cnt[r] = 0;
+            }
+            since_flush = 0;
         }
     }
     __syncthreads();

@@ -249,6 +249,22 @@ inline ResidentPlan resident_plan(int L, int n_rep, int sm_count)
     }
 }
 
+// can a cluster of `cs` CTAs be scheduled at all on the current device? (ising3d_set_cluster_size)
+inline cudaError_t resident_try_size(int L, int cs, int n_rep, int *clusters)
+{
+    const size_t smem = resident_smem_bytes(L, cs);
+    auto prep = [](auto kernel) {
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    };
+    switch (L) {
+        case 64:  prep(resident_sweep_kernel<1>); return resident_try<1>(cs, n_rep, smem, clusters);
+        case 128: prep(resident_sweep_kernel<2>); return resident_try<2>(cs, n_rep, smem, clusters);
+        case 256: prep(resident_sweep_kernel<4>); return resident_try<4>(cs, n_rep, smem, clusters);
+        default:  return cudaErrorInvalidValue;
+    }
+}
+
 template <int WPR>
 inline cudaError_t launch_resident_t(uint32_t *state, const uint64_t *d_seeds, int n_rep,
                                      const ResidentPlan &plan, uint32_t t0, uint32_t n_sweeps,

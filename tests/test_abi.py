@@ -87,6 +87,52 @@ def test_bad_arguments_return_einval(lib):
     assert lib.ising3d_last_error() is not None
 
 
+def test_concurrent_callers_keep_their_own_errors(lib):
+    """include/ising3d.h: distinct handles are independent, ising3d_last_error is thread-local.
+    Eight host threads validate / try to create handles at the same time (no process-wide launch
+    plan or attribute cache is left to race on): every thread sees its own error text, *h stays
+    untouched, nothing crashes."""
+    import threading
+    from paper_2305_12161_b200 import binding
+    bad = [(100, b"multiple of 64"), (32, b"multiple of 64"), (8192, b"multiple of 64")]
+    errors, gate = [], threading.Barrier(8)
+
+    def worker(i):
+        try:
+            gate.wait()
+            for rep in range(200):
+                L, text = bad[(i + rep) % len(bad)]
+                h = C.c_void_p()
+                if (i + rep) % 2:
+                    rc = lib.ising3d_init(C.byref(h), L, i)
+                    assert rc == binding.EINVAL and h.value is None
+                    assert text in lib.ising3d_last_error()
+                else:
+                    rc = lib.ising3d_sweep(None, 1)
+                    assert rc == binding.EINVAL and b"null handle" in lib.ising3d_last_error()
+                assert lib.ising3d_required_bytes(64 * (1 + i), 1 + rep % 3) > 0
+        except BaseException as e:   # noqa: BLE001
+            errors.append((i, repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(8)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
+def test_no_process_wide_launch_state_in_the_library():
+    """The launch plans and function-attribute flags live in the handle (struct ising3d), not in
+    function-local statics two handles could race on."""
+    csrc = os.path.join(ROOT, "paper_2305_12161_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        txt = re.sub(r"//.*", "", open(os.path.join(csrc, f)).read())
+        for m in re.finditer(r"^\s+static\s+(?!constexpr|const\b|_assert|assert)[^;(]*;", txt, flags=re.M):
+            raise AssertionError("%s: mutable function-local static: %s" % (f, m.group(0).strip()))
+        assert "getenv" not in txt, f
+
+
 def test_no_cpu_fallback(lib):
     """Without a CUDA device the library must refuse to compute (ECUDA/ENOMEM), never emulate."""
     import torch

@@ -163,6 +163,27 @@ def test_menger_full_size_structure(B, orc):
     sim.free()
 
 
+def test_menger_k0_at_L2048_tile_index_beyond_32_bits(B, orc):
+    """k = 0 at L = 2048: one tile per site, tile index T = (z*L + y)*L + x up to 2^33 (D11).
+    Sampled sites (both halves in z, so that a tile index truncated to 32 bits would alias
+    planes z and z + 1024) against the oracle's single-site form of the rule."""
+    L, seed = 2048, 4
+    sim = B.Ising3D(L, [seed])
+    sim.init_menger(0)
+    buf = np.empty(L ** 3 // 32, dtype=np.uint32)
+    words = sim.get_state(buf)
+    rng = np.random.Generator(np.random.PCG64(5))
+    xyz = rng.integers(0, L, size=(3000, 3)).astype(np.int32)
+    mirror = xyz.copy()
+    mirror[:, 2] = (mirror[:, 2] + L // 2) % L
+    xyz = np.concatenate([xyz, mirror, [[0, 0, 0], [L - 1, L - 1, L - 1], [0, 0, L // 2]]]).astype(np.int32)
+    got = _bits_at(words, L, xyz)
+    want = np.array([orc.menger_site(seed, L, 0, int(x), int(y), int(z)) for x, y, z in xyz], dtype=np.int8)
+    assert np.array_equal(got, want)
+    assert (xyz[:, 2] >= L // 2).sum() > 1000        # tile indices >= 2^32 are covered
+    sim.free()
+
+
 # ------------------------------------------------------------------ f-4 (part): L = 4096 on one GPU
 def test_L4096_one_gpu(B, orc):
     """The size the paper hopes for next ("L=4096, in the near future"): 6.9e10 spins,

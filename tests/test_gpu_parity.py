@@ -87,11 +87,11 @@ def test_generic_kernel_other_sizes(B, orc, L, seed, cps):
 @pytest.mark.parametrize("L,cs,seed,cps", [(64, 1, 1, [1, 2, 5, 10]), (64, 2, 1, [3, 10]), (64, 8, 21, [1, 7]),
                                            (64, 16, 22, [2, 5]), (128, 2, 7, [1, 2, 5, 12]), (128, 4, 7, [3, 12]),
                                            (128, 8, 23, [1, 6]), (128, 16, 24, [4]), (256, 16, 2, [1, 3, 10])])
-def test_resident_kernel_cluster_sizes(B, orc, L, cs, seed, cps, monkeypatch):
+def test_resident_kernel_cluster_sizes(B, orc, L, cs, seed, cps):
     """The shared-memory-resident multi-sweep kernel at every cluster size (z slabs of L/cs
     planes, halo planes exchanged through distributed shared memory), against the oracle."""
-    monkeypatch.setenv("ISING3D_RESIDENT_CS", str(cs))
     sim = B.Ising3D(L, [seed], variant=B.VARIANT_RESIDENT)
+    sim.set_cluster_size(cs)
     assert sim.variant_name == "resident" and sim.cluster_size == cs
     ref = orc.Oracle(L, seed)
     t = 0
@@ -304,6 +304,37 @@ def test_config3_batch_equals_singles_and_oracle(B, orc, variant):
         one.free()
 
 
+@pytest.mark.slow
+def test_config3_four_replicas_all_10000_sweeps_in_one_call(B, orc):
+    """the batch of 64 x L = 128 runs ALL 10^4 sweeps through one
+    ising3d_sweep(10^4) call (the resident kernel: one launch), and replicas 100, 101, 131, 163
+    are followed by the oracle to the end: every word and every count."""
+    from concurrent.futures import ThreadPoolExecutor
+    L, n = 128, 10_000
+    seeds = inputs.WORKLOADS["config3_64xL128"]["seeds"]
+    picked = (100, 101, 131, 163)
+    batch = B.Ising3D(L, seeds)
+    assert batch.variant_name == "resident" and batch.n_rep == 64
+    l0 = batch.launch_count
+    batch.sweep(n)
+    assert batch.launch_count - l0 == 1 and batch.sweep_count == n
+    st = batch.get_state().reshape(64, L ** 3 // 32)
+    meas = batch.measure()
+
+    def follow(seed):
+        orc.set_num_threads(max(1, (os.cpu_count() or 4) // len(picked)))
+        ref = orc.Oracle(L, seed)
+        ref.sweep(n)
+        return seed, ref.export_words(), ref.measure_full()
+
+    with ThreadPoolExecutor(len(picked)) as pool:
+        for seed, words, want in pool.map(follow, picked):
+            assert np.array_equal(st[seed - 100], words), "replica %d differs at t = %d" % (seed, n)
+            check_measure(meas, want, rep=seed - 100)
+    orc.set_num_threads(os.cpu_count() or 4)
+    batch.free()
+
+
 @pytest.mark.parametrize("L,variant,name", [(512, "auto", "fused2"), (1024, "fused3", "fused3"),
                                             (256, "fused", "fused")])
 def test_large_L_batch_equals_singles(B, orc, L, variant, name):
@@ -412,6 +443,50 @@ def test_checkpoint_resume_and_reset(B, orc):
         s.free()
 
 
+@pytest.mark.parametrize("L,n_sweeps", [(512, 3), (64, 20), (256, 5)])
+def test_two_handles_two_streams_two_threads(B, orc, L, n_sweeps):
+    """include/ising3d.h: "distinct handles are independent".  Two host threads each create a
+    handle of the SAME L on their own stream and drive it at the same time (the first sweep of
+    each builds that handle's launch plan concurrently); each must match the oracle bit for bit."""
+    import threading
+    import torch
+    seeds = (41, 42)
+    gate = threading.Barrier(2)
+    out, errors = {}, []
+
+    def worker(i):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                gate.wait()
+                sim = B.Ising3D(L, [seeds[i]])
+                gate.wait()
+                for _ in range(n_sweeps):
+                    sim.sweep(1)
+                m = sim.measure()
+                out[i] = (sim.get_state(), m)
+                sim.free()
+        except BaseException as e:   # noqa: BLE001
+            errors.append((i, repr(e)))
+            try:
+                gate.abort()
+            except Exception:
+                pass
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for i, seed in enumerate(seeds):
+        ref = orc.Oracle(L, seed)
+        ref.sweep(n_sweeps)
+        assert np.array_equal(out[i][0], ref.export_words()), "handle %d differs" % i
+        check_measure(out[i][1], ref.measure_full())
+
+
 def test_library_owned_memory_and_errors(B, orc):
     sim = B.Ising3D(64, [1], torch_buffer=False)
     with pytest.raises(B.Ising3DError):
@@ -486,8 +561,9 @@ def test_measure_variant_errors(B):
 
 
 # ------------------------------------------------------------------ configs 4 and 5: windows at full size
-@pytest.mark.parametrize("name,t_enter,n_window", [("config4_L1024", 1000, 4), ("config4_L1024", 99_996, 4),
-                                                   ("config5_L2048", 1000, 2)])
+@pytest.mark.parametrize("name,t_enter,n_window", [
+    ("config4_L1024", 1000, 4), ("config4_L1024", 99_996, 4), ("config5_L2048", 1000, 2),
+    pytest.param("config5_L2048", 299_998, 2, marks=pytest.mark.slow)])   # the end of the full run
 def test_full_size_window_against_oracle(B, orc, name, t_enter, n_window):
     """the oracle cannot follow 10^5 sweeps of L = 1024 or anything long at
     L = 2048, but the RNG is counter based, so a window entered through get_state is exact:
@@ -506,8 +582,15 @@ def test_full_size_window_against_oracle(B, orc, name, t_enter, n_window):
     ref.sweep(n_window)
     assert sim.sweep_count == ref.sweep_count == t_enter + n_window
     assert np.array_equal(sim.get_state(buf), ref.export_words()), "window state differs"
-    thin = np.array([0, 1, 2, 3, 5, 8, 16, 33, 64, 128, 257, L // 4, L // 2 - 1, L // 2] if L <= 1024
-                    else [0, 1, 2, 3, 16, 257, L // 2 - 1, L // 2], dtype=np.int32)
+    if L <= 1024:
+        # {1..8, 16, 32, ..., 512} plus 16 seeded-random r
+        rng = np.random.Generator(np.random.PCG64(2305_12161))
+        extra = rng.choice(np.arange(9, L // 2), size=16, replace=False)
+        thin = np.unique(np.concatenate([np.arange(0, 9), 2 ** np.arange(4, 10), extra,
+                                         [L // 4, L // 2 - 1, L // 2]])).astype(np.int32)
+        assert thin.size >= 30 and thin.max() == L // 2
+    else:
+        thin = np.array([0, 1, 2, 3, 16, 257, L // 2 - 1, L // 2], dtype=np.int32)
     got = sim.measure()
     n_up, a = ref.measure(thin)
     assert int(got["n_up"][0]) == n_up

@@ -172,6 +172,36 @@ def test_init_menger_tile_signs_fair():
     assert set(np.unique(tiles)) <= {13, -13}
 
 
+def test_menger_site_equals_the_array_form_and_the_documented_bit_beyond_2_to_32():
+    """orc_menger_site (one site of D11) against orc_init_menger site by site on small lattices,
+    and, where the tile index T passes 2^32 (L = 2048, k = 0: T = (z*L + y)*L + x up to 2^33),
+    against the rule written out with the big-integer Python Philox: sign bit = bit T & 31 of
+    word (T >> 5) & 3 of Philox(counter (T >> 7 mod 2^32, k, 0, 3)) (D11)."""
+    for L, k, seed in [(20, 1, 9), (18, 2, 10), (12, 0, 11)]:
+        o = orc.Oracle(L, seed, init=False)
+        o.init_menger(k)
+        s = o.spins
+        for z in range(L):
+            for y in range(L):
+                for x in range(0, L, 1 if L < 16 else 3):
+                    assert orc.menger_site(seed, L, k, x, y, z) == int(s[z, y, x])
+    L, seed = 2048, 4
+    key = [seed & MASK, seed >> 32]
+    seen_high = 0
+    for (x, y, z) in [(0, 0, 0), (5, 0, 1023), (7, 1, 1024), (2047, 2047, 2047), (100, 900, 1500),
+                      (100, 900, 476), (1, 2, 2046), (64, 0, 1024), (64, 0, 0)]:
+        T = (z * L + y) * L + x
+        seen_high += T >= 2 ** 32
+        word = py_philox([(T >> 7) & MASK, 0, 0, 3], key)[(T >> 5) & 3]
+        want = 1 if (word >> (T & 31)) & 1 else -1
+        assert orc.menger_site(seed, L, 0, x, y, z) == want, (x, y, z)
+    assert seen_high >= 4
+    # a 32-bit tile index would alias planes z and z + 1024 at L = 2048: the rule does not
+    a = [orc.menger_site(seed, L, 0, x, 3, 10) for x in range(256)]
+    b = [orc.menger_site(seed, L, 0, x, 3, 10 + 1024) for x in range(256)]
+    assert a != b
+
+
 # ------------------------------------------------------------------ f-1: FFT correlation + radial average
 def _exact_bin(L, dx, dy, dz):
     """D12 restated with exact rationals: nearest integer to |d| of the minimal image."""
