@@ -72,7 +72,9 @@ extern "C" {
 #define ISING3D_ECUDA  (-3)   /* CUDA runtime error; text in ising3d_last_error()         */
 
 /* sweep-kernel variants (ising3d_set_variant) */
-#define ISING3D_VARIANT_AUTO    0   /* resident (L <= 256), fused2 (L in 512..4096), else generic */
+#define ISING3D_VARIANT_AUTO    0   /* resident (L <= 256), fused2 (L in 512..4096; switches to the
+                                       activity-driven kernel when few groups can still change,
+                                       see ising3d_set_activity_policy), else generic           */
 #define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
 #define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
 #define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096); a batch
@@ -82,6 +84,12 @@ extern "C" {
 #define ISING3D_VARIANT_FUSED3  5   /* two sweeps per launch, the state in between stays in shared
                                        memory (L in {1024, 2048}, 01 cycle); an odd last sweep and
                                        the mixed cycle run on fused2                           */
+
+#define ISING3D_VARIANT_ACTIVE  6   /* activity-driven: only the 128-spin groups that hold a site with
+                                       Delta E <= 0, or that read a word changed since their last
+                                       evaluation, are evaluated (two launches per sweep, in place;
+                                       L in {256,512,1024,2048,4096}, plain checkerboard, T = 0).
+                                       Same trajectory; pays once few groups can change        */
 
 /* measurement kernels (ising3d_set_measure_variant) */
 #define ISING3D_MEASURE_AUTO     0  /* tensor where the shape allows (L % 512 == 0), else popcount */
@@ -211,6 +219,38 @@ int ising3d_set_stream(ising3d_t *h, void *cuda_stream);
 int ising3d_set_variant(ising3d_t *h, int variant);
 
 /*
+ * Activity of the state (eq. (6): a site can change only if Delta E <= 0, i.e.
+ * n >= 3 of its six neighbours are antiparallel).  awake_groups: HOST [n_rep][2] or NULL; entry
+ * [rep][c] = number of 128-spin groups (the Philox groups q of D5) of colour c that hold at least
+ * one site with n >= 3 in the current state -- an exact integer, a function of the state only.
+ * last_fraction: HOST or NULL; with awake_groups the fraction of such groups (both colours, all
+ * replicas), without it the fraction seen by the last probe of the AUTO policy (-1 if none yet).
+ * Counting needs L in {256,512,1024,2048,4096} (EINVAL otherwise) and synchronises the stream.
+ */
+int ising3d_activity(ising3d_t *h, uint64_t *awake_groups, double *last_fraction);
+
+/*
+ * Work done by the activity-driven kernel since the last call (or since the handle was created):
+ * evaluated_changed HOST [n_rep][2] = 128-spin groups evaluated (both colours, all sweeps) and
+ * groups whose words changed.  A diagnostic of the kernel, not of the state: evaluated groups are
+ * the ones holding a Delta E <= 0 site plus the ones woken by a neighbour's change.  Resets the
+ * tallies; synchronises the stream.  EINVAL unless L in {256,512,1024,2048,4096}.
+ */
+int ising3d_active_stats(ising3d_t *h, uint64_t *evaluated_changed);
+
+/*
+ * Policy of ISING3D_VARIANT_AUTO at L >= 512 (T = 0, plain checkerboard): after every
+ * `probe_interval` sweeps the activity flags are rebuilt and counted; if the
+ * fraction of groups that can change is below `on_below` the following sweeps run on the
+ * activity-driven kernel, which hands back to fused2 if the same fraction, probed every
+ * probe_interval sweeps, passes `off_above`.  The choice changes the speed only, never the
+ * result.  probe_interval = 0: always fused2.  Defaults: 1024, 0.075, 0.10 (measured break-even
+ * of the two kernels at L = 2048).
+ * Each probe / check synchronises the stream once.  EINVAL unless 0 <= on_below <= off_above <= 1.
+ */
+int ising3d_set_activity_policy(ising3d_t *h, uint64_t probe_interval, double on_below, double off_above);
+
+/*
  * Thread-block cluster size of the resident kernel (L in {64,128,256}): the lattice is split
  * into `cs` z slabs, one CTA (= one SM) each, halo planes exchanged through distributed shared
  * memory after every half-sweep.  cs = 0 restores the automatic choice (the
@@ -222,7 +262,8 @@ int ising3d_set_cluster_size(ising3d_t *h, int cs);
 
 /*
  * Run n_sweeps checkerboard sweeps (eq. (6)).
- * Asynchronous on the handle's stream; no host synchronisation inside.
+ * Asynchronous on the handle's stream; no host synchronisation inside, except the one per
+ * probe_interval sweeps of the AUTO policy at L >= 512 (ising3d_set_activity_policy).
  * The sweep counter advances by n_sweeps; EINVAL if it would pass 2^32-1.
  */
 int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);

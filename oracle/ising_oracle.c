@@ -32,6 +32,8 @@
  *   orc_postprocess     : closed forms, hand-worked example
  *   orc_export/import   : round trip, independent Python packer
  *   orc_site_after      : equals orc_sweep site by site on small L
+ *   orc_activity        : all up -> 0, Neel -> all groups, one reversed spin -> one group,
+ *                         equals "some tie-bit assignment changes the group" by brute force
  *   orc_first_colour / orc_sweep_mixed : Neel state closed form (the first colour
  *                         decides the sign of the ordered state), bit statistics,
  *                         big-integer Python Philox
@@ -255,6 +257,46 @@ void orc_sweep(orc_t *o, uint64_t n_sweeps)
         orc_half_sweep(o, o->sweep, 1, 0, 0);
         o->sweep += 1;
     }
+}
+
+/* ------------------------------------------------------------------ */
+/* Activity of a state (what ising3d_activity counts).  eq. (6)        */
+/* PAPER.md:105-108 changes a site only if Delta E <= 0, Delta E =     */
+/* 2 s_i sum_nn s_j.  out[c] = number of 128-spin groups */
+/* q = b>>7 (D3/D5) of colour c that hold at least one site with       */
+/* Delta E <= 0 in the current configuration.  A function of the       */
+/* state only; no random numbers.                                      */
+/* Pins: all up -> 0; Neel -> every group; one reversed spin -> 1      */
+/* group of its colour, 0 of the other; a group counts iff a half-     */
+/* sweep with some tie-bit assignment could change it (checked         */
+/* against orc_half_sweep with both seeds' bits on small L).           */
+/* ------------------------------------------------------------------ */
+void orc_activity(const orc_t *o, uint64_t out[2])
+{
+    const int L = o->L;
+    const uint64_t groups = ((uint64_t)L * L * (L / 2) + 127u) >> 7;   /* per colour */
+    uint8_t *mark = (uint8_t *)calloc(2 * groups, 1);
+    for (int z = 0; z < L; ++z)
+        for (int y = 0; y < L; ++y)
+            for (int x = 0; x < L; ++x) {
+                int h = o->s[orc_idx(o, orc_mod(x + 1, L), y, z)]
+                      + o->s[orc_idx(o, orc_mod(x - 1, L), y, z)]
+                      + o->s[orc_idx(o, x, orc_mod(y + 1, L), z)]
+                      + o->s[orc_idx(o, x, orc_mod(y - 1, L), z)]
+                      + o->s[orc_idx(o, x, y, orc_mod(z + 1, L))]
+                      + o->s[orc_idx(o, x, y, orc_mod(z - 1, L))];
+                int dE = 2 * (int)o->s[orc_idx(o, x, y, z)] * h;
+                if (dE <= 0) {
+                    int c = (x + y + z) & 1;
+                    mark[(uint64_t)c * groups + (orc_bit_index(L, x, y, z) >> 7)] = 1;
+                }
+            }
+    out[0] = out[1] = 0;
+    for (uint64_t g = 0; g < groups; ++g) {
+        out[0] += mark[g];
+        out[1] += mark[groups + g];
+    }
+    free(mark);
 }
 
 /* ------------------------------------------------------------------ */

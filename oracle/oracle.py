@@ -88,6 +88,8 @@ def lib():
         l.orc_sites_after.argtypes = [C.c_uint64, C.c_int, i32p, C.c_int, C.c_int,
                                       C.POINTER(C.c_int8)]
         l.orc_sites_after.restype = None
+        l.orc_activity.argtypes = [C.c_void_p, u64p]
+        l.orc_activity.restype = None
         l.orc_first_colour.argtypes = [C.c_uint64, C.c_uint32]
         l.orc_first_colour.restype = C.c_int
         l.orc_sweep_mixed.argtypes = [C.c_void_p, C.c_uint64]
@@ -359,6 +361,12 @@ class Oracle:
     def half_sweep_T(self, t: int, c: int, T: float):
         thr = glauber_thresholds(T)
         self._l.orc_half_sweep_T(self._h, int(t), int(c), _p(thr, C.c_uint64))
+
+    def activity(self) -> np.ndarray:
+        """[2]: groups of each colour holding a site with Delta E <= 0 (eq. (6))."""
+        out = np.zeros(2, dtype=np.uint64)
+        self._l.orc_activity(self._h, _p(out, C.c_uint64))
+        return out
 
     def sweep_mixed(self, n: int = 1):
         """n sweeps of the mixed cycle (D10): the first colour is drawn per sweep."""

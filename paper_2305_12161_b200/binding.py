@@ -21,6 +21,7 @@ CYCLE_01, CYCLE_MIXED, CYCLE_DOUBLE_CB, CYCLE_DOUBLE_CB_MIXED = 0, 1, 2, 3
 MEASURE_AUTO, MEASURE_POPCOUNT, MEASURE_TENSOR = 0, 1, 2
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_FUSED, VARIANT_FUSED2, VARIANT_RESIDENT = 0, 1, 2, 3, 4
 VARIANT_FUSED3 = 5
+VARIANT_ACTIVE = 6
 
 EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
@@ -29,7 +30,7 @@ EXPORTED = [
     "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
     "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size",
-    "ising3d_set_cluster_size", "ising3d_sync",
+    "ising3d_set_cluster_size", "ising3d_activity", "ising3d_active_stats", "ising3d_set_activity_policy", "ising3d_sync",
     "ising3d_free", "ising3d_last_error",
 ]
 
@@ -97,6 +98,9 @@ def load():
         "ising3d_variant_name": (C.c_char_p, [vp]),
         "ising3d_cluster_size": (C.c_int, [vp]),
         "ising3d_set_cluster_size": (C.c_int, [vp, C.c_int]),
+        "ising3d_activity": (C.c_int, [vp, u64p, C.POINTER(C.c_double)]),
+        "ising3d_active_stats": (C.c_int, [vp, u64p]),
+        "ising3d_set_activity_policy": (C.c_int, [vp, u64, C.c_double, C.c_double]),
         "ising3d_sync": (C.c_int, [vp]),
         "ising3d_free": (None, [vp]),
         "ising3d_last_error": (C.c_char_p, []),
@@ -186,6 +190,28 @@ class Ising3D:
 
     def set_cluster_size(self, cs: int):
         _check(self._l.ising3d_set_cluster_size(self._h, int(cs)))
+
+    def set_activity_policy(self, probe_interval: int, on_below: float = 0.075, off_above: float = 0.10):
+        _check(self._l.ising3d_set_activity_policy(self._h, int(probe_interval), float(on_below), float(off_above)))
+
+    def activity(self):
+        """(awake_groups [n_rep][2], fraction): groups holding a site with Delta E <= 0."""
+        out = np.zeros((self.n_rep, 2), dtype=np.uint64)
+        frac = C.c_double()
+        _check(self._l.ising3d_activity(self._h, out.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(frac)))
+        return out, float(frac.value)
+
+    def active_stats(self) -> np.ndarray:
+        """[n_rep][2]: groups evaluated / changed by the activity-driven kernel since the last call."""
+        out = np.zeros((self.n_rep, 2), dtype=np.uint64)
+        _check(self._l.ising3d_active_stats(self._h, out.ctypes.data_as(C.POINTER(C.c_uint64))))
+        return out
+
+    @property
+    def last_activity(self) -> float:
+        frac = C.c_double()
+        _check(self._l.ising3d_activity(self._h, None, C.byref(frac)))
+        return float(frac.value)
 
     def set_measure_variant(self, variant: int):
         _check(self._l.ising3d_set_measure_variant(self._h, variant))

@@ -17,6 +17,7 @@
 #include "kernels_fused.cuh"
 #include "kernels_fused2.cuh"
 #include "kernels_fused3.cuh"
+#include "kernels_active.cuh"
 #include "kernels_generic.cuh"
 #include "kernels_fft.cuh"
 #include "kernels_gram.cuh"
@@ -80,6 +81,17 @@ struct ising3d {
     // kernel (nothing process-wide: distinct handles are independent, include/ising3d.h)
     ising::FusedPlan plan_f1, plan_f2, plan_f3;
     bool attr_gram = false, attr_autocorr = false;
+    // activity-driven sweeps (kernels_active.cuh): one flag per 128-spin group and colour
+    uint32_t *d_awake = nullptr;               // [n_rep][2][G/32]; valid only while flags_valid
+    unsigned long long *d_act = nullptr;       // [n_rep][4]: flag counts of colour 0, 1; groups evaluated, changed
+    unsigned int *d_tickets = nullptr;         // work-item counter of active_halfsweep_kernel (never reset)
+    ising::ActivePlan plan_act;
+    bool flags_valid = false;                  // the flags describe state[cur] (set by activity_flags, kept by active sweeps)
+    bool active_mode = false;                  // AUTO: the activity-driven kernel is the one being dispatched
+    uint64_t run_len = 0;                      // sweeps since the last probe / check (AUTO)
+    uint64_t probe_interval = 1024;            // AUTO: dense sweeps between two activity probes (0 = never)
+    double active_on = 0.075, active_off = 0.10;   // AUTO: switch on below / off above this awake fraction
+    double last_activity = -1.0;               // awake fraction seen by the last probe / check
 
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
@@ -114,6 +126,24 @@ struct ising3d {
         return variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3 ||
                (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
+    bool active_ok() const { return ising::active_supported(L); }
+    bool use_active() const      // forced; AUTO switches to it by itself (sweep_auto)
+    {
+        return variant == ISING3D_VARIANT_ACTIVE && cycle <= ISING3D_CYCLE_MIXED && temperature == 0.0;
+    }
+    bool auto_adaptive() const
+    {
+        return variant == ISING3D_VARIANT_AUTO && fused2_ok() && active_ok() && cycle <= ISING3D_CYCLE_MIXED &&
+               temperature == 0.0 && probe_interval > 0;
+    }
+    void state_changed()         // the state was replaced: flags and the adaptive history are void
+    {
+        flags_valid = false;
+        active_mode = false;
+        run_len = 0;
+        last_activity = -1.0;
+    }
+    size_t flag_words() const { return (size_t)L * L * (L >> 8) / 32; }   // per colour
     bool use_fused() const
     {
         if (cycle != ISING3D_CYCLE_01) return false;
@@ -125,7 +155,7 @@ struct ising3d {
 namespace {
 
 struct Layout {
-    size_t state, seeds, counts, gsum, queue, total;
+    size_t state, seeds, counts, gsum, queue, awake, act, total;
 };
 
 Layout make_layout(int L, int n_rep)
@@ -136,7 +166,10 @@ Layout make_layout(int L, int n_rep)
     l.counts = align_up((size_t)n_rep * (1 + 3 * (L / 2 + 1)) * 8, 256);
     l.gsum = align_up((size_t)n_rep * 3 * (L / 2 + 1) * 8, 256);
     l.queue = align_up((size_t)n_rep * 3 * 4, 256);
-    l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue;
+    const bool act = ising::active_supported(L);
+    l.awake = act ? align_up((size_t)n_rep * 2 * ((size_t)L * L * (L >> 8) / 8), 256) : 0;
+    l.act = act ? align_up((size_t)n_rep * 4 * 8, 256) + 256 : 0;        // + the ticket counter
+    l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue + l.awake + l.act;
     return l;
 }
 
@@ -148,6 +181,7 @@ int launch_init(ising3d *h)
     h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     h->sweep = 0;
+    h->state_changed();
     return ISING3D_OK;
 }
 
@@ -192,12 +226,22 @@ int create(ising3d_t **out, int L, int n_rep, const uint64_t *seeds, void *dev_b
         h->d_counts = (unsigned long long *)(p + 2 * lay.state + lay.seeds);
         h->d_gsum = (unsigned long long *)(p + 2 * lay.state + lay.seeds + lay.counts);
         h->d_queue = (unsigned int *)(p + 2 * lay.state + lay.seeds + lay.counts + lay.gsum);
+        if (lay.awake) {
+            h->d_awake = (uint32_t *)(p + 2 * lay.state + lay.seeds + lay.counts + lay.gsum + lay.queue);
+            h->d_act = (unsigned long long *)(p + 2 * lay.state + lay.seeds + lay.counts + lay.gsum +
+                                              lay.queue + lay.awake);
+            h->d_tickets = (unsigned int *)((char *)h->d_act + lay.act - 256);
+        }
         int dev = 0;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
             (e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev)) !=
                 cudaSuccess ||
             (e = cudaMemcpyAsync(h->d_seeds, h->seeds.data(), (size_t)n_rep * 8,
                                  cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) {
+            code = fail(ISING3D_ECUDA, std::string("setup: ") + cudaGetErrorString(e));
+            break;
+        }
+        if (h->d_act && (e = cudaMemsetAsync(h->d_act, 0, lay.act, h->stream)) != cudaSuccess) {
             code = fail(ISING3D_ECUDA, std::string("setup: ") + cudaGetErrorString(e));
             break;
         }
@@ -284,7 +328,8 @@ int sweep_resident(ising3d *h, uint64_t n)
 
 // One launch per replica and sweep (pair of sweeps for fused3): the replicas of a batch are
 // independent lattices at a stride of words_per_replica() in both ping-pong buffers.
-int sweep_fused(ising3d *h, uint64_t n, bool gen2)
+// Runs the sweeps with indices h->sweep + i0 .. h->sweep + i0 + n - 1.
+int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
 {
     const size_t wpr = h->words_per_replica();
     uint64_t i = 0;
@@ -297,12 +342,13 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
         if (e != cudaSuccess)
             return fail(ISING3D_ECUDA, std::string("fused sweep plan: ") + cudaGetErrorString(e));
     }
+    if (n) h->flags_valid = false;             // the dense kernels do not keep the activity flags
     // pairs of sweeps with the intermediate state on chip (01 cycle); an odd last sweep below
     for (; gen2 && h->use_fused3() && i + 2 <= n; i += 2) {
         for (int rep = 0; rep < h->n_rep; ++rep) {
             cudaError_t e = ising::launch_fused3_sweep2(
                 h->state[h->cur] + rep * wpr, h->state[1 - h->cur] + rep * wpr, h->L,
-                (uint32_t)(h->sweep + i), h->seeds[rep], h->plan_f3, h->stream);
+                (uint32_t)(h->sweep + i0 + i), h->seeds[rep], h->plan_f3, h->stream);
             if (e != cudaSuccess)
                 return fail(ISING3D_ECUDA, std::string("fused3 sweep launch: ") + cudaGetErrorString(e));
         }
@@ -310,7 +356,7 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
         h->launches += h->n_rep;
     }
     for (; i < n; ++i) {
-        const uint32_t t = (uint32_t)(h->sweep + i);
+        const uint32_t t = (uint32_t)(h->sweep + i0 + i);
         for (int rep = 0; rep < h->n_rep; ++rep) {
             const uint64_t seed = h->seeds[rep];
             const uint32_t *src = h->state[h->cur] + rep * wpr;
@@ -328,6 +374,100 @@ int sweep_fused(ising3d *h, uint64_t n, bool gen2)
         h->launches += h->n_rep;
     }
     CUDA_TRY(cudaGetLastError());
+    return ISING3D_OK;
+}
+
+// Activity flags of state[cur] (kernels_active.cuh): flag = the group holds a site with Delta E <= 0
+// (eq. (6)).  Counts land in d_act[rep][0..1].
+int build_flags(ising3d *h)
+{
+    const size_t wpr = h->words_per_replica(), fw = h->flag_words();
+    CUDA_TRY(cudaMemset2DAsync(h->d_act, 4 * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][0..1]
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        cudaError_t e = ising::launch_activity_flags(h->state[h->cur] + rep * wpr, h->d_awake + rep * 2 * fw,
+                                                     h->d_act + rep * 4, h->L, h->stream);
+        if (e != cudaSuccess)
+            return fail(ISING3D_ECUDA, std::string("activity flags launch: ") + cudaGetErrorString(e));
+    }
+    h->launches += h->n_rep;
+    h->flags_valid = true;
+    return ISING3D_OK;
+}
+
+// Synchronises the stream.  frac = mean over replicas and colours of d_act[rep][0..1] / G;
+// raw[rep][0..1] = the two counts.
+int read_activity(ising3d *h, double *frac, uint64_t *raw)
+{
+    std::vector<unsigned long long> host((size_t)h->n_rep * 4);
+    CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_act, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    const double G = (double)h->flag_words() * 32.0;
+    double sum = 0.0;
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        sum += (double)host[rep * 4 + 0] + (double)host[rep * 4 + 1];
+        if (raw) {
+            raw[rep * 2 + 0] = host[rep * 4 + 0];
+            raw[rep * 2 + 1] = host[rep * 4 + 1];
+        }
+    }
+    if (frac) *frac = sum / (2.0 * G * h->n_rep);
+    return ISING3D_OK;
+}
+
+// Sweeps h->sweep + i0 .. + n - 1 on the activity-driven kernels, in place in state[cur].
+int sweep_active(ising3d *h, uint64_t i0, uint64_t n)
+{
+    if (n == 0) return ISING3D_OK;
+    if (!h->flags_valid) {
+        const int rc = build_flags(h);
+        if (rc != ISING3D_OK) return rc;
+    }
+    if (!h->plan_act.ready) {
+        cudaError_t e = ising::plan_active(h->plan_act, h->L, h->sm_count);
+        if (e != cudaSuccess) return fail(ISING3D_ECUDA, std::string("active sweep plan: ") + cudaGetErrorString(e));
+    }
+    const size_t wpr = h->words_per_replica(), fw = h->flag_words();
+    for (uint64_t i = 0; i < n; ++i) {
+        const uint32_t t = (uint32_t)(h->sweep + i0 + i);
+        for (int rep = 0; rep < h->n_rep; ++rep) {
+            const uint64_t seed = h->seeds[rep];
+            const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
+            cudaError_t e = ising::launch_active_sweep(h->state[h->cur] + rep * wpr, h->d_awake + rep * 2 * fw,
+                                                       h->d_act + rep * 4 + 2, h->d_tickets, h->plan_act,
+                                                       h->L, t, seed, first, h->stream);
+            if (e != cudaSuccess)
+                return fail(ISING3D_ECUDA, std::string("active sweep launch: ") + cudaGetErrorString(e));
+        }
+        h->launches += 2 * (uint64_t)h->n_rep;
+    }
+    return ISING3D_OK;
+}
+
+// ISING3D_VARIANT_AUTO at L >= 512, T = 0, plain checkerboard: dense fused2 sweeps while most groups
+// still hold a site that can change, the activity-driven kernel once few do.  Every probe_interval
+// sweeps the flags are rebuilt and counted (one stream synchronisation); below active_on the next
+// sweeps run activity-driven, and go back to fused2 if the fraction passes active_off.
+int sweep_auto(ising3d *h, uint64_t n)
+{
+    uint64_t i = 0;
+    while (i < n) {
+        const uint64_t m = std::min<uint64_t>(n - i, h->probe_interval - h->run_len);
+        int rc = h->active_mode ? sweep_active(h, i, m) : sweep_fused(h, i, m, true);
+        if (rc != ISING3D_OK) return rc;
+        i += m;
+        h->run_len += m;
+        if (h->run_len < h->probe_interval) break;
+        // the same probe in both modes: rebuild the flags (exact: the ones an active run carries also
+        // hold woken groups not evaluated yet) and count the groups that hold a Delta E <= 0 site
+        double frac = 0.0;
+        rc = build_flags(h);
+        if (rc == ISING3D_OK) rc = read_activity(h, &frac, nullptr);
+        if (rc != ISING3D_OK) return rc;
+        if (h->active_mode && frac > h->active_off) h->active_mode = false;
+        else if (!h->active_mode && frac < h->active_on) h->active_mode = true;
+        h->last_activity = frac;
+        h->run_len = 0;
+    }
     return ISING3D_OK;
 }
 
@@ -538,6 +678,8 @@ int ising3d_set_cycle(ising3d_t *h, int cycle)
     if (cycle >= ISING3D_CYCLE_DOUBLE_CB &&
         (h->variant == ISING3D_VARIANT_FUSED2 || h->variant == ISING3D_VARIANT_FUSED3))
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+    if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_ACTIVE)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     h->cycle = cycle;
     return ISING3D_OK;
 }
@@ -555,14 +697,19 @@ int ising3d_init_menger(ising3d_t *h, int k)
     h->launches += 1;
     CUDA_TRY(cudaGetLastError());
     h->sweep = 0;
+    h->state_changed();
     return ISING3D_OK;
 }
 
 int ising3d_set_variant(ising3d_t *h, int variant)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
-    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_FUSED3)
+    if (variant < ISING3D_VARIANT_AUTO || variant > ISING3D_VARIANT_ACTIVE)
         return fail(ISING3D_EINVAL, "unknown variant");
+    if (variant == ISING3D_VARIANT_ACTIVE && !h->active_ok())
+        return fail(ISING3D_EINVAL, "the activity-driven kernel needs L in {256,512,1024,2048,4096}");
+    if (variant == ISING3D_VARIANT_ACTIVE && h->cycle >= ISING3D_CYCLE_DOUBLE_CB)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
         variant != ISING3D_VARIANT_GENERIC)
         return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
@@ -580,6 +727,53 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (variant == ISING3D_VARIANT_RESIDENT && !h->resident_ok())
         return fail(ISING3D_EINVAL, "resident kernel needs L in {64,128,256} and a cluster that fits");
     h->variant = variant;
+    h->active_mode = false;
+    h->run_len = 0;
+    return ISING3D_OK;
+}
+
+int ising3d_set_activity_policy(ising3d_t *h, uint64_t probe_interval, double on_below, double off_above)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (!(on_below >= 0.0) || !(off_above >= on_below) || !(off_above <= 1.0))
+        return fail(ISING3D_EINVAL, "need 0 <= on_below <= off_above <= 1");
+    h->probe_interval = probe_interval;
+    h->active_on = on_below;
+    h->active_off = off_above;
+    h->active_mode = false;
+    h->run_len = 0;
+    return ISING3D_OK;
+}
+
+int ising3d_activity(ising3d_t *h, uint64_t *awake_groups, double *last_fraction)
+{
+    if (!h) return fail(ISING3D_EINVAL, "null handle");
+    if (last_fraction) *last_fraction = h->last_activity;
+    if (!awake_groups) return ISING3D_OK;
+    if (!h->active_ok()) return fail(ISING3D_EINVAL, "activity counts need L in {256,512,1024,2048,4096}");
+    // Counting rebuilds the flags from the state: the flags an active run carries are a superset
+    // (woken groups not yet evaluated), the rebuilt ones are exact and satisfy the same invariant.
+    int rc = build_flags(h);
+    if (rc != ISING3D_OK) return rc;
+    double frac = 0.0;
+    rc = read_activity(h, &frac, awake_groups);
+    if (rc != ISING3D_OK) return rc;
+    if (last_fraction) *last_fraction = frac;
+    return ISING3D_OK;
+}
+
+int ising3d_active_stats(ising3d_t *h, uint64_t *evaluated_changed)
+{
+    if (!h || !evaluated_changed) return fail(ISING3D_EINVAL, "null pointer");
+    if (!h->active_ok()) return fail(ISING3D_EINVAL, "the activity-driven kernel needs L in {256,512,1024,2048,4096}");
+    std::vector<unsigned long long> host((size_t)h->n_rep * 4);
+    CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_act, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(cudaMemset2DAsync(h->d_act + 2, 4 * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][2..3]
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        evaluated_changed[rep * 2 + 0] = host[rep * 4 + 2];
+        evaluated_changed[rep * 2 + 1] = host[rep * 4 + 3];
+    }
     return ISING3D_OK;
 }
 
@@ -611,10 +805,13 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps)
     if (h->sweep + n_sweeps > 0xFFFFFFFFull || h->sweep + n_sweeps < h->sweep)
         return fail(ISING3D_EINVAL, "sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return ISING3D_OK;
+    if (!h->auto_adaptive() && !h->use_active()) h->flags_valid = false;   // kernels that do not keep the flags
     const int rc = h->temperature > 0.0 ? sweep_glauber(h, n_sweeps)
                    : h->use_resident() ? sweep_resident(h, n_sweeps)
-                   : h->use_fused2()  ? sweep_fused(h, n_sweeps, true)
-                   : h->use_fused() ? sweep_fused(h, n_sweeps, false)
+                   : h->use_active()   ? sweep_active(h, 0, n_sweeps)
+                   : h->auto_adaptive() ? sweep_auto(h, n_sweeps)
+                   : h->use_fused2()  ? sweep_fused(h, 0, n_sweeps, true)
+                   : h->use_fused() ? sweep_fused(h, 0, n_sweeps, false)
                                     : sweep_generic(h, n_sweeps);
     if (rc != ISING3D_OK) return rc;
     h->sweep += n_sweeps;
@@ -786,6 +983,7 @@ int ising3d_set_state(ising3d_t *h, const uint32_t *words, size_t n_words, uint6
     CUDA_TRY(cudaMemcpyAsync(h->state[h->cur], words, n_words * 4, cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     h->sweep = sweep;
+    h->state_changed();
     return ISING3D_OK;
 }
 
@@ -809,6 +1007,7 @@ int ising3d_set_state_device(ising3d_t *h, const uint32_t *dev_words, size_t n_w
     CUDA_TRY(cudaMemcpyAsync(h->state[h->cur], dev_words, n_words * 4, cudaMemcpyDeviceToDevice,
                              h->stream));
     h->sweep = sweep;
+    h->state_changed();
     return ISING3D_OK;
 }
 
@@ -826,6 +1025,7 @@ const char *ising3d_variant_name(const ising3d_t *h)
 {
     if (!h) return "none";
     if (h->temperature > 0.0) return "glauber";
+    if (h->use_active() || (h->auto_adaptive() && h->active_mode && !h->use_resident())) return "active";
     return h->use_resident() ? "resident" : h->use_fused3() ? "fused3" : h->use_fused2() ? "fused2" : h->use_fused() ? "fused" : "generic";
 }
 

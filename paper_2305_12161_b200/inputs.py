@@ -114,6 +114,19 @@ def coarse_words(L: int, seed: int, block: int = 8) -> np.ndarray:
     return pack_spins(s)
 
 
+def domain_spins(L: int, seed: int, block: int = 16, p_minority: float = 0.15, noise: float = 0.0) -> np.ndarray:
+    """A late-time-like state as int8 spins: a +1 background in which a fraction p_minority of
+    the block^3 cubes is -1 (large uniform regions, activity only at the cube edges and
+    corners), optionally with a fraction `noise` of the sites flipped."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    nb = L // block
+    coarse = np.where(rng.random((nb, nb, nb)) < p_minority, -1, 1).astype(np.int8)
+    s = np.kron(coarse, np.ones((block, block, block), dtype=np.int8))
+    if noise > 0.0:
+        s = np.where(rng.random((L, L, L)) < noise, -s, s).astype(np.int8)
+    return s
+
+
 # ----------------------------------------------------------------------
 # structured configurations (closed-form test inputs)
 # ----------------------------------------------------------------------

@@ -1,0 +1,211 @@
+"""GPU parity of the activity-driven sweep (kernels_active.cuh, ISING3D_VARIANT_ACTIVE and the
+AUTO policy) and of ising3d_activity, against the CPU oracle: the trajectory must be the dense
+kernels' bit for bit (eq. (6) PAPER.md:105-108 leaves a group without a Delta E <= 0 site
+unchanged whatever its random bits are), and the activity count is an exact integer."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2305_12161_b200 import inputs  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2305_12161_b200 import build, binding
+    build.build()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    oracle.build()
+    return oracle
+
+
+def _states(L):
+    """(name, packed words): an iid start, late-time-like domain states, structured states."""
+    return [
+        ("domains16", inputs.pack_spins(inputs.domain_spins(L, 5, block=16, p_minority=0.15))),
+        ("domains32_noise", inputs.pack_spins(inputs.domain_spins(L, 6, block=32, p_minority=0.3, noise=0.002))),
+        ("coarse8", inputs.coarse_words(L, 3)),
+        ("cube", inputs.pack_spins(inputs.cube(L, L - 1, L - 1, L - 1, 2))),      # across all three wraps
+        ("slab", inputs.pack_spins(inputs.slab(L, 0, L - 3, 7))),                 # flat interfaces normal to x
+        ("all_up", inputs.pack_spins(inputs.all_up(L))),
+    ]
+
+
+def test_activity_counts_equal_oracle(B, orc):
+    """ising3d_activity == orc_activity (groups holding a Delta E <= 0 site, per colour)."""
+    L = 256
+    G = L ** 3 // 256
+    sim = B.Ising3D(L, [2])
+    ref = orc.Oracle(L, 2)
+    for t in (0, 3, 20):
+        sim.sweep(t - sim.sweep_count)
+        ref.sweep(t - ref.sweep_count)
+        got, frac = sim.activity()
+        want = ref.activity()
+        assert list(got[0]) == list(want), "t=%d" % t
+        assert abs(frac - (int(want[0]) + int(want[1])) / (2.0 * G)) < 1e-15
+        assert np.array_equal(sim.get_state(), ref.export_words())       # counting changes nothing
+    seen = []
+    for name, words in _states(L):
+        sim.set_state(words, 100)
+        ref.import_words(words, 100)
+        got, _ = sim.activity()
+        want = ref.activity()
+        assert list(got[0]) == list(want), name
+        seen.append(int(want[0]) + int(want[1]))
+    assert seen[-1] == 0 and min(seen[:-2]) > 0 and max(seen) < 2 * G      # non-trivial counts
+    sim.free()
+
+
+@pytest.mark.parametrize("cycle", ["01", "mixed"])
+def test_active_sweep_against_oracle_L256(B, orc, cycle):
+    """The activity-driven kernel from the T = infinity start (every group awake) and from
+    late-time-like states (few groups awake), every checkpoint against the oracle."""
+    L = 256
+    sim = B.Ising3D(L, [9], variant=B.VARIANT_ACTIVE)
+    assert sim.variant_name == "active"
+    if cycle == "mixed":
+        sim.set_cycle(B.CYCLE_MIXED)
+    ref = orc.Oracle(L, 9)
+    step = ref.sweep if cycle == "01" else ref.sweep_mixed
+    for cp in (1, 2, 5, 12):
+        sim.sweep(cp - sim.sweep_count)
+        step(cp - ref.sweep_count)
+        assert np.array_equal(sim.get_state(), ref.export_words()), "random start, sweep %d" % cp
+    for name, words in _states(L):
+        sim.set_state(words, 1000)
+        ref.import_words(words, 1000)
+        for cp in (1001, 1002, 1005, 1012, 1030):
+            sim.sweep(cp - sim.sweep_count)
+            step(cp - ref.sweep_count)
+            assert np.array_equal(sim.get_state(), ref.export_words()), "%s, sweep %d" % (name, cp)
+    got, want = sim.measure(), ref.measure_full()
+    assert int(got["n_up"][0]) == want["n_up"] and np.array_equal(got["antipar"][0], want["antipar"])
+    sim.free()
+
+
+def test_active_sweep_against_oracle_L512_batch(B, orc):
+    """Rows of two groups (x-edge wake-ups cross groups), two replicas in one handle."""
+    L = 512
+    seeds = [31, 32]
+    sim = B.Ising3D(L, seeds, variant=B.VARIANT_ACTIVE)
+    w0 = inputs.pack_spins(inputs.domain_spins(L, 7, block=32, p_minority=0.2, noise=0.001))
+    w1 = inputs.coarse_words(L, 8, block=16)
+    sim.set_state(np.concatenate([w0, w1]), 500)
+    refs = [orc.Oracle(L, s, init=False) for s in seeds]
+    refs[0].import_words(w0, 500)
+    refs[1].import_words(w1, 500)
+    for cp in (501, 503, 508):
+        sim.sweep(cp - sim.sweep_count)
+        got = sim.get_state().reshape(2, -1)
+        for r in range(2):
+            refs[r].sweep(cp - refs[r].sweep_count)
+            assert np.array_equal(got[r], refs[r].export_words()), "replica %d, sweep %d" % (r, cp)
+    cnt, _ = sim.activity()
+    for r in range(2):
+        assert list(cnt[r]) == list(refs[r].activity())
+    sim.free()
+
+
+def test_auto_policy_switches_and_keeps_the_trajectory(B, orc):
+    """AUTO at L = 512 with a short probe interval: a late-time-like state switches to the
+    activity-driven kernel, an iid state stays on fused2, and either way the states equal the
+    oracle's; interleaving dense and activity-driven sweeps (flags rebuilt) changes nothing."""
+    L = 512
+    sim = B.Ising3D(L, [41])
+    sim.set_activity_policy(4, 0.5, 0.9)
+    assert sim.variant_name == "fused2" and sim.last_activity == -1.0
+    ref = orc.Oracle(L, 41)
+    sim.sweep(9)                                   # iid start: probes at 4 and 8 see every group awake
+    ref.sweep(9)
+    assert sim.variant_name == "fused2" and sim.last_activity > 0.9
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    words = inputs.pack_spins(inputs.domain_spins(L, 11, block=32, p_minority=0.2, noise=0.0005))
+    sim.set_state(words, 200)
+    ref.import_words(words, 200)
+    assert sim.variant_name == "fused2"            # set_state voids the history
+    sim.sweep(3)
+    assert sim.variant_name == "fused2"
+    sim.sweep(3)                                   # the probe after sweep 4 switches; 2 active sweeps follow
+    assert sim.variant_name == "active" and 0.0 < sim.last_activity < 0.5
+    ref.sweep(6)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    sim.sweep(11)
+    ref.sweep(11)
+    assert sim.variant_name == "active"
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    # forced dense, then AUTO again (the flags are rebuilt at the next probe)
+    sim.set_variant(B.VARIANT_FUSED2)
+    sim.sweep(2)
+    sim.set_variant(B.VARIANT_AUTO)
+    assert sim.variant_name == "fused2"
+    sim.sweep(7)
+    ref.sweep(9)
+    assert sim.variant_name == "active"
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    got, want = sim.measure(), ref.measure_full()
+    assert int(got["n_up"][0]) == want["n_up"] and np.array_equal(got["antipar"][0], want["antipar"])
+    # handing back: an iid state set into an active handle goes dense again
+    sim.set_state(inputs.random_words(L, 1, 5), 0)
+    sim.sweep(4)
+    assert sim.variant_name == "fused2"
+    sim.free()
+
+
+def test_auto_policy_disabled_and_bad_arguments(B):
+    sim = B.Ising3D(512, [1])
+    sim.set_activity_policy(0)
+    sim.set_state(inputs.pack_spins(inputs.all_up(512)), 0)
+    sim.sweep(5)
+    assert sim.variant_name == "fused2"
+    with pytest.raises(B.Ising3DError):
+        sim.set_activity_policy(4, 0.5, 0.4)
+    with pytest.raises(B.Ising3DError):
+        sim.set_activity_policy(4, -0.1, 0.4)
+    sim.free()
+    small = B.Ising3D(128, [1])
+    with pytest.raises(B.Ising3DError):
+        small.set_variant(B.VARIANT_ACTIVE)
+    with pytest.raises(B.Ising3DError):
+        small.activity()
+    small.free()
+
+
+@pytest.mark.slow
+def test_active_equals_fused2_at_full_size_late_time(B, orc):
+    """Config 5 (L = 2048, seed 4) taken to t = 10^4 on fused2, then 24 sweeps on the
+    activity-driven kernel against 24 more fused2 sweeps: every word equal; then two sweeps from
+    the t0 state against the whole-lattice oracle, and the activity count."""
+    import torch
+    L, seed, t0, n = 2048, 4, 10000, 24
+    a = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED2)
+    a.sweep(t0)
+    nw = L ** 3 // 32
+    buf = torch.empty(nw, dtype=torch.int32, device="cuda")
+    a.get_state_device(buf.data_ptr(), nw)
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_ACTIVE)
+    b.set_state_device(buf.data_ptr(), nw, t0)
+    cnt, frac = b.activity()
+    assert 0.05 < frac < 0.6
+    a.sweep(n)
+    b.sweep(n)
+    wa, wb = a.get_state(), b.get_state()
+    assert np.array_equal(wa, wb)
+    del wa, wb
+    # two sweeps from the t0 state against the whole-lattice oracle (8.6 GB of int8 spins)
+    ref = orc.Oracle(L, seed, init=False)
+    ref.import_words(buf.cpu().numpy().view(np.uint32), t0)
+    ref.sweep(2)
+    b.set_state_device(buf.data_ptr(), nw, t0)
+    b.sweep(2)
+    assert np.array_equal(b.get_state(), ref.export_words())
+    assert list(b.activity()[0][0]) == list(ref.activity())
+    a.free()
+    b.free()

@@ -539,3 +539,60 @@ def test_dcb_mixed_python_restatement_and_invariants():
     keep = a.spins.copy()
     a.sweep_dcb_mixed(3, block=4)
     assert np.array_equal(a.spins, keep)
+
+
+# ------------------------------------------------------------------ activity (ising3d_activity)
+def _groups_changed(before: np.ndarray, after: np.ndarray) -> np.ndarray:
+    """[2][groups] bool: 128-spin groups (4 packed words, D3) whose words differ."""
+    d = (before != after).reshape(2, -1, 4).any(axis=2)
+    return d
+
+
+def test_activity_closed_forms():
+    """eq. (6): only sites with Delta E <= 0 can change.  All up: none.  Neel
+    state: every site has Delta E = -12, so every group counts.  One reversed spin in an ordered
+    lattice: that site has Delta E = -12, its six neighbours Delta E = +8: exactly one group, of
+    the reversed site's colour."""
+    L = 16
+    G = L ** 3 // 2 // 128
+    o = orc.Oracle(L, 1, init=False)
+    o.spins[...] = 1
+    assert list(o.activity()) == [0, 0]
+    o.spins[...] = inputs.neel(L)
+    assert list(o.activity()) == [G, G]
+    for (x, y, z) in [(0, 0, 0), (5, 2, 8), (15, 15, 15), (3, 0, 15)]:
+        o.spins[...] = -1
+        o.spins[z, y, x] = 1
+        want = [0, 0]
+        want[(x + y + z) & 1] = 1
+        assert list(o.activity()) == want
+
+
+@pytest.mark.parametrize("L,kind,sweeps", [(16, "random", 0), (32, "random", 6), (64, "domains", 0),
+                                           (64, "domains", 4), (64, "noisy", 0), (64, "noisy", 1)])
+def test_activity_is_exactly_the_groups_a_half_sweep_can_change(L, kind, sweeps):
+    """Operational pin through the separately pinned orc_half_sweep: from one configuration, the
+    union over many seeds (= tie-bit assignments) of the groups a colour-c half-sweep changes is
+    exactly the set of groups holding a site with Delta E <= 0 -- a site with Delta E < 0 flips
+    for every seed, a tie for about half of them -- and the count is non-trivial (neither 0 nor
+    all groups) on the domain states."""
+    base = orc.Oracle(L, 77)
+    if kind == "domains":
+        base.spins[...] = inputs.domain_spins(L, 5, block=16, p_minority=0.15)
+    elif kind == "noisy":
+        base.spins[...] = inputs.domain_spins(L, 6, block=16, p_minority=0.3, noise=0.002)
+    base.sweep(sweeps)
+    words0 = base.export_words()
+    spins0 = base.spins.copy()
+    want = base.activity()
+    G = L ** 3 // 2 // 128
+    union = np.zeros((2, G), dtype=bool)
+    for seed in range(200, 248):                       # 48 tie-bit assignments: a miss has p = 2^-48
+        for c in (0, 1):
+            o = orc.Oracle(L, seed, init=False)
+            o.spins[...] = spins0
+            o.half_sweep(sweeps, c)
+            union[c] |= _groups_changed(words0, o.export_words())[c]
+    assert [int(union[0].sum()), int(union[1].sum())] == [int(want[0]), int(want[1])]
+    if kind != "random":
+        assert 0 < want[0] < G and 0 < want[1] < G
