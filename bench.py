@@ -46,6 +46,10 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-measure", action="store_true", help="step = reset + sweeps only")
+    ap.add_argument("--no-late-windows", action="store_true",
+                    help="skip the sweeps-only windows at t = 10^4 and 10^5 of the full run (about 40 s)")
+    ap.add_argument("--cpu-sizes", default="256x20,1024x2,2048x1",
+                    help="extra oracle timings LxSWEEPS (SURVEY.md 8(d)); empty to skip")
     return ap.parse_args()
 
 
@@ -123,6 +127,33 @@ def oracle_rate(L: int, n_sweeps: int, seed: int):
     o.sweep(n_sweeps)
     dt = time.perf_counter() - t0
     return (L ** 3) * n_sweeps / dt / 1e9, dt, orc.num_threads()
+
+
+def oracle_sizes(spec: str):
+    """the oracle timed at L=256 x 20, L=1024 x 2, L=2048 x 1 sweeps (the last one
+    only with >= 16 GiB of free host RAM), plus its single-thread rate (L=256 x 4)."""
+    from oracle import oracle as orc
+    out = []
+    try:
+        import psutil
+        free_gib = psutil.virtual_memory().available / 2 ** 30
+    except Exception:
+        free_gib = 0.0
+    for item in [x for x in spec.split(",") if x]:
+        L, n = (int(v) for v in item.split("x"))
+        if L ** 3 / 2 ** 30 * 1.5 > free_gib or (L >= 2048 and free_gib < 16):
+            out.append({"L": L, "sweeps": n, "skipped": "%.0f GiB of host RAM free" % free_gib})
+            continue
+        rate, dt, cores = oracle_rate(L, n, 4)
+        out.append({"L": L, "sweeps": n, "value": rate, "unit": UNIT, "cores": cores, "seconds": dt})
+    cores = orc.num_threads()
+    orc.set_num_threads(1)
+    try:
+        rate, dt, _ = oracle_rate(256, 4, 4)
+    finally:
+        orc.set_num_threads(cores)
+    single = {"L": 256, "sweeps": 4, "value": rate, "unit": UNIT, "cores": 1, "seconds": dt}
+    return out, single
 
 
 def run_reference(args):
@@ -266,6 +297,7 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop()
     launches = sim.launch_count - launches0
+    timed_kernel = sim.variant_name            # the sweep kernel of the timed steps
     total_ms = e0.elapsed_time(e1)
     init_ms = sum(t[0].elapsed_time(t[1]) for t in timers) / args.steps
     sweep_ms = sum(t[1].elapsed_time(t[2]) for t in timers) / args.steps
@@ -302,6 +334,31 @@ def run_ours(args):
                "ms_per_step": ems / k_e2e,
                "note": "set_state(pinned host, 1 GiB at L=2048) + sweep + measure(host counts) per step"}
 
+    # ---------------- sweeps-only windows of the full run ----------------
+    # t = 0 is the headline window above; the lattice is then taken on to t = 10^4 and 10^5 (AUTO policy:
+    # fused2, handing over to the activity-driven kernel once few groups can still change) and `wS` sweeps
+    # are timed at each, with the fraction of 128-spin groups that hold a Delta E <= 0 site.
+    windows = [{"t0": 0, "sweeps": S, "ms_per_sweep": sweep_ms / S, "kernel": timed_kernel,
+                "site_updates_per_ns": N / (sweep_ms / S * 1e6), "awake_group_fraction": 1.0 if L >= 256 else None}]
+    if not args.no_late_windows and world == 1:
+        sim.reset()
+        wS = 200
+        for t0 in (10_000, 100_000):
+            sim.sweep(t0 - sim.sweep_count)
+            try:
+                frac = sim.activity()[1]
+            except Exception:
+                frac = None
+            sim.sync()
+            w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            w0.record()
+            sim.sweep(wS)
+            w1.record()
+            torch.cuda.synchronize()
+            ms = w0.elapsed_time(w1) / wS
+            windows.append({"t0": t0, "sweeps": wS, "ms_per_sweep": ms, "kernel": sim.variant_name,
+                            "site_updates_per_ns": N / (ms * 1e6), "awake_group_fraction": frac})
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -310,9 +367,9 @@ def run_ours(args):
     # ---------------- roofline of the dominant kernel (the sweep kernel) ----------------
     peak, peak_src, peaks = measured_peak()
     kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel",
-              "fused3": "fused3_sweep2_kernel"}.get(sim.variant_name, "halfsweep_generic_kernel")
+              "fused3": "fused3_sweep2_kernel"}.get(timed_kernel, "halfsweep_generic_kernel")
     # fused3: one launch = two sweeps (an odd last sweep of a step runs on fused2; S is even here)
-    launches_per_sweep = {"fused": 1, "fused2": 1, "fused3": 0.5}.get(sim.variant_name, 2)
+    launches_per_sweep = {"fused": 1, "fused2": 1, "fused3": 0.5}.get(timed_kernel, 2)
     avg_launch_ms = sweep_ms / (S * launches_per_sweep)
     algo_bytes_per_launch = ALGO_BYTES_PER_SITE_UPDATE * N / launches_per_sweep
     achieved = algo_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
@@ -324,15 +381,31 @@ def run_ours(args):
     alu_ops_per_site = 69.0 / 128.0
     alu_bound = 148 * 64 * sm_mhz * 1e6 / alu_ops_per_site / 1e9
     hbm_bound = peak / ALGO_BYTES_PER_SITE_UPDATE
+    sweep_rate = N * S / (sweep_ms * 1e6)
+    traffic = ncu_traffic(kernel, L)
+    # as compiled (profiles/r1i, ncu smsp__inst_executed.sum): 337 warp-instructions per thread-step of
+    # 4 groups = 512 sites, 60 of 64 tile rows and 256 of 260 planes stored
+    compiled_per_site = 337.0 / 512.0 * (64.0 / 60.0) * (260.0 / 256.0)
+    compiled_bound = 148 * 64 * sm_mhz * 1e6 / compiled_per_site / 1e9
     roofline = {
         "bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": achieved / peak, "traffic": ncu_traffic(kernel, L),
+        "frac": achieved / peak, "traffic": traffic,
+        # what binds the kernel is the issue rate of its integer instructions, not HBM:
+        "binding_limit": "issue",
+        "issue_frac": sweep_rate / alu_bound,
+        "issue_frac_as_compiled": sweep_rate / compiled_bound if kernel == "fused2_sweep_kernel" else None,
+        "issue_model": {"thread_instr_per_clk_per_sm": 64, "sms": 148, "sm_mhz": sm_mhz,
+                        "min_instr_per_128_sites_per_colour": 69,
+                        "compiled_warp_instr_per_thread_step_of_512_sites": 337,
+                        "source": "microbench/pipe_rates.cu, microbench/sweep_ceiling.cu; profiles/r1c, r1h, r1i"},
+        # on the bytes the kernel really moves (ncu dram__bytes_read + write per launch)
+        "frac_on_bytes_moved": (traffic / (avg_launch_ms * 1e-3) / 1e9) / peak if traffic else None,
         "algorithmic_bytes_per_launch": algo_bytes_per_launch, "avg_launch_ms": avg_launch_ms,
         "peak_source": peak_src,
-        "sweep_only_site_updates_per_ns": N * S / (sweep_ms * 1e6),
+        "sweep_only_site_updates_per_ns": sweep_rate,
         "hbm_bound_site_updates_per_ns": hbm_bound,
         "alu_bound_site_updates_per_ns": alu_bound,
-        "frac_of_min_roofline": (N * S / (sweep_ms * 1e6)) / min(hbm_bound, alu_bound),
+        "frac_of_min_roofline": sweep_rate / min(hbm_bound, alu_bound),
         # the stricter view: the N/4 bytes per sweep a fused black+white pass cannot avoid moving
         "frac_on_fused_floor_bytes": (0.25 * N / launches_per_sweep / (avg_launch_ms * 1e-3) / 1e9) / peak
         if launches_per_sweep <= 1 else None,
@@ -347,6 +420,8 @@ def run_ours(args):
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "L=%d, iid p=1/2 start from seed 4, sweeps 0..%d (%.1f s of CPU work); "
                          "same rule and RNG as config 5, smaller box" % (Lc, nsw - 1, dt)}
+        if args.cpu_sizes:
+            cpu["other_sizes"], cpu["single_thread"] = oracle_sizes(args.cpu_sizes)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -355,11 +430,12 @@ def run_ours(args):
         "config": {"workload": "config5_L2048: L=%d periodic cube, iid p=1/2 start from seed %d, "
                                "step = reset + %d zero-T checkerboard sweeps + measure(r<=%d)" % (
                                    L, seed, S, L // 2),
-                   "L": L, "sweeps_per_step": S, "replicas_per_gpu": 1, "kernel": sim.variant_name,
+                   "L": L, "sweeps_per_step": S, "replicas_per_gpu": 1, "kernel": timed_kernel,
                    "l2": "inputs larger than L2 (%.0f MiB packed lattice, ping-pong; L2 126 MB)" % (
                        N / 8 / 2 ** 20),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "breakdown_ms": {"init": init_ms, "sweeps": sweep_ms, "measure": meas_ms},
+        "windows": windows,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roofline, "cpu_baseline": cpu,
         "result": None if last is None else {"sweep": last["sweep"], "n_up": int(last["n_up"][0]),

@@ -187,14 +187,15 @@ int ising3d_init_menger(ising3d_t *h, int k);
  * (coarse colour (x/8 + y/8 + z/8) mod 2); a sweep updates the red blocks (their darker sites,
  * (x+y+z) even, then their lighter sites) with everything else frozen, then the blue blocks:
  * four masked half-sweeps, every spin proposed once, tie bits as in the plain checkerboard.
- * Runs on the resident (L <= 256) and generic kernels.  Its mixed cycle (Table I;
+ * Runs on the resident (L <= 256), fused2 (L in 512..4096: one masked launch per coarse colour,
+ * dark then light sites inside it) and generic kernels.  Its mixed cycle (Table I;
  * reading D15): the coarse colour updated first in sweep t is the D10 bit; block
  * Bi = (bz*nB + by)*nB + bx (nB = L/8) updates first the fine colour given by bit (Bi & 127) of
  * Philox(key = seed, counter = (Bi >> 7, t, 0, 36)), then the other; generic kernel only (the
  * block bits of a sweep are drawn into the handle's idle state buffer).  Takes effect from the
  * next sweep.
  * EINVAL for an unknown value, with ISING3D_VARIANT_FUSED (01 cycle only), for the double
- * checkerboard with ISING3D_VARIANT_FUSED2, or at T > 0 for anything but the 01 cycle.
+ * checkerboard with ISING3D_VARIANT_FUSED3 or _ACTIVE, or at T > 0 for anything but the 01 cycle.
  */
 int ising3d_set_cycle(ising3d_t *h, int cycle);
 

@@ -122,7 +122,7 @@ struct ising3d {
     bool use_fused3() const { return variant == ISING3D_VARIANT_FUSED3 && cycle == ISING3D_CYCLE_01; }
     bool use_fused2() const
     {
-        if (cycle >= ISING3D_CYCLE_DOUBLE_CB) return false;     // masked phases: resident / generic
+        if (cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED) return false;   // per-block orders: generic kernel
         return variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3 ||
                (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
@@ -363,15 +363,28 @@ int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
             uint32_t *dst = h->state[1 - h->cur] + rep * wpr;
             // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
             const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
-            cudaError_t e =
-                gen2 ? ising::launch_fused2_sweep(src, dst, h->L, t, seed, first, h->plan_f2, h->stream)
-                     : ising::launch_fused_sweep(src, dst, h->L, t, ising::make_philox_keys(seed),
-                                                 h->plan_f1, h->stream);
+            cudaError_t e;
+            if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
+                // D14: the red blocks (dark, then light sites), then the blue blocks: two masked
+                // launches, src -> dst -> src
+                e = ising::launch_fused2_sweep(src, dst, h->L, t, seed, 0, h->plan_f2, h->stream, 0);
+                if (e == cudaSuccess)
+                    e = ising::launch_fused2_sweep(dst, const_cast<uint32_t *>(src), h->L, t, seed, 0,
+                                                   h->plan_f2, h->stream, 1);
+            } else {
+                e = gen2 ? ising::launch_fused2_sweep(src, dst, h->L, t, seed, first, h->plan_f2, h->stream)
+                         : ising::launch_fused_sweep(src, dst, h->L, t, ising::make_philox_keys(seed),
+                                                     h->plan_f1, h->stream);
+            }
             if (e != cudaSuccess)
                 return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
         }
-        h->cur = 1 - h->cur;
-        h->launches += h->n_rep;
+        if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
+            h->launches += 2 * (uint64_t)h->n_rep;         // back in state[cur]
+        } else {
+            h->cur = 1 - h->cur;
+            h->launches += h->n_rep;
+        }
     }
     CUDA_TRY(cudaGetLastError());
     return ISING3D_OK;
@@ -675,9 +688,8 @@ int ising3d_set_cycle(ising3d_t *h, int cycle)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     if (cycle != ISING3D_CYCLE_01 && h->variant == ISING3D_VARIANT_FUSED)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
-    if (cycle >= ISING3D_CYCLE_DOUBLE_CB &&
-        (h->variant == ISING3D_VARIANT_FUSED2 || h->variant == ISING3D_VARIANT_FUSED3))
-        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+    if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED3)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
     if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_ACTIVE)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     h->cycle = cycle;
@@ -713,9 +725,8 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
         variant != ISING3D_VARIANT_GENERIC)
         return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
-    if ((variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3) &&
-        h->cycle == ISING3D_CYCLE_DOUBLE_CB)
-        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+    if (variant == ISING3D_VARIANT_FUSED3 && h->cycle == ISING3D_CYCLE_DOUBLE_CB)
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
     if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())

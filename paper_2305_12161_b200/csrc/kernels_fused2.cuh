@@ -157,10 +157,20 @@ struct F2Ctx {
 // U = position of the step in the 6-step unrolled march (k = 6 lap + U).  With a ring of 3 or 6 stages
 // the stage of the step, and with it every shared-memory address, is base + immediate; the mbarrier
 // parity is U/3 (S = 3) or the parity of the lap (S = 6).  The exchange plane index is U & 1.
-template <int R4, int PLANE, int U>
+// DCB (double checkerboard, Supp. I.A PAPER.md:223-240, D14): only the sites of one coarse colour are
+// updated in this launch; mB / mW are the bit masks of those sites in the words of this thread's two
+// rows (same block row) at the black plane z and at the white plane z-1; the other sites keep their
+// old value (they are the frozen halo of the blocks being updated).
+__device__ __forceinline__ uint4 keep_unmasked(const uint4 upd, const uint4 old, const uint32_t m)
+{
+    return make_uint4((upd.x & m) | (old.x & ~m), (upd.y & m) | (old.y & ~m), (upd.z & m) | (old.z & ~m),
+                      (upd.w & m) | (old.w & ~m));
+}
+
+template <int R4, int PLANE, int U, bool DCB>
 __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const uint32_t qb,
                                         const uint32_t qw, const uint32_t lap_parity,
-                                        const SweepConsts &keys)
+                                        const SweepConsts &keys, const uint32_t mB, const uint32_t mW)
 {
     constexpr int S = kF2Stages;
     constexpr int PH = U % 3, O = U & 1;
@@ -185,6 +195,10 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
         const uint4 Wx1 = xneigh<1 - O>(w.W[Z][1], c.lane_prev, c.lane_next);
         w.B[P][0] = rule_group(Bo0, rho0, w.W[Z][0], Wx0, Wym, w.W[Z][1], w.W[M][0], w.W[P][0]);
         w.B[P][1] = rule_group(Bo1, rho1, w.W[Z][1], Wx1, w.W[Z][0], Wyp, w.W[M][1], w.W[P][1]);
+        if (DCB) {
+            w.B[P][0] = keep_unmasked(w.B[P][0], Bo0, mB);
+            w.B[P][1] = keep_unmasked(w.B[P][1], Bo1, mB);
+        }
         uint4 *nbw = c.nb + O * PLANE + c.si0;
         nbw[0] = w.B[P][0];
         nbw[R4] = w.B[P][1];
@@ -203,10 +217,12 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
         const uint4 rho1 = philox_folded<1>(q + R4, keys);
         const uint4 Bx0 = xneigh<O>(w.B[Z][0], c.lane_prev, c.lane_next);
         const uint4 Bx1 = xneigh<1 - O>(w.B[Z][1], c.lane_prev, c.lane_next);
-        const uint4 nW0 =
-            rule_group(w.W[M][0], rho0, w.B[Z][0], Bx0, Bym, w.B[Z][1], w.B[M][0], w.B[P][0]);
-        const uint4 nW1 =
-            rule_group(w.W[M][1], rho1, w.B[Z][1], Bx1, w.B[Z][0], Byp, w.B[M][1], w.B[P][1]);
+        uint4 nW0 = rule_group(w.W[M][0], rho0, w.B[Z][0], Bx0, Bym, w.B[Z][1], w.B[M][0], w.B[P][0]);
+        uint4 nW1 = rule_group(w.W[M][1], rho1, w.B[Z][1], Bx1, w.B[Z][0], Byp, w.B[M][1], w.B[P][1]);
+        if (DCB) {
+            nW0 = keep_unmasked(nW0, w.W[M][0], mW);
+            nW1 = keep_unmasked(nW1, w.W[M][1], mW);
+        }
         if (k >= 4) {
             uint4 *d = c.dstW + (size_t)q;
             if (c.ok0) d[0] = nW0;
@@ -218,10 +234,12 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
 // Grid: blockIdx.x = y tile (RPT stored rows each, RPT even), blockIdx.y = z chunk.
 // Chunk boundaries are odd planes, so the first marched plane z0 = zs-3 is even and the
 // in-row direction of the even tile row at step k is k & 1.
-template <int R4, int NT>
+// DCB: `coarse` = the coarse colour updated by this launch (a double-checkerboard sweep is the launch
+// for coarse 0 followed by the one for coarse 1, each dark sites then light sites, D14).
+template <int R4, int NT, bool DCB>
 __global__ void __launch_bounds__(NT, 2)
 fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, const int L,
-                    const int RPT, const int nzc, const int first,
+                    const int RPT, const int nzc, const int first, const int coarse,
                     const __grid_constant__ SweepConsts keys)
 {
     constexpr int TY = 2 * NT / R4;    // rows in the tile (incl. 2+2 halo rows)
@@ -328,11 +346,19 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     // plane z-1 (qw = the previous step's qb), kept incrementally
     uint32_t qb = (uint32_t)z * c.qplane + c.qrow;
     uint32_t qw = (uint32_t)(z == 0 ? L - 1 : z - 1) * c.qplane + c.qrow;
+    // double checkerboard: bits j of a word with ((j >> 2) + (y >> 3) + (z >> 3)) & 1 == coarse (philox.cuh)
+    const uint32_t ycoarse = DCB ? (uint32_t)((y >> 3) + coarse) : 0u;
+    uint32_t mB = 0xFFFFFFFFu, mW = 0xFFFFFFFFu;
 
 #define F2_STEP(U)                                                            \
     {                                                                         \
         if (k >= K) break;                                                    \
-        f2_step<R4, PLANE, U>(w, c, k, qb, qw, lap_parity, keys);             \
+        if (DCB) {                                                            \
+            const int zw = z == 0 ? L - 1 : z - 1;                            \
+            mB = ((ycoarse + (uint32_t)(z >> 3)) & 1u) ? 0xF0F0F0F0u : 0x0F0F0F0Fu;  \
+            mW = ((ycoarse + (uint32_t)(zw >> 3)) & 1u) ? 0xF0F0F0F0u : 0x0F0F0F0Fu; \
+        }                                                                     \
+        f2_step<R4, PLANE, U, DCB>(w, c, k, qb, qw, lap_parity, keys, mB, mW); \
         __syncthreads();                                                      \
         if (prod_warp && pk < K) issue_next();                                \
         ++k;                                                                  \
@@ -362,11 +388,17 @@ inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
     constexpr int TY = 2 * NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
-    cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT>,
+    cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, true>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT>, NT, smem);
+    int occ = 0, occ_dcb = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT, false>, NT, smem);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_dcb, fused2_sweep_kernel<R4, NT, true>, NT, smem);
+    if (occ_dcb < occ) occ = occ_dcb;          // one launch shape for both
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     const int tyo = TY - 4;                        // stored rows per tile (even)
@@ -385,16 +417,21 @@ inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
 }
 
 template <int R4, int NT>
-inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first,
+inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first, int coarse,
                                    const SweepConsts &keys, const FusedPlan &plan, cudaStream_t stream)
 {
     constexpr int TY = 2 * NT / R4;
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
     dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
-    fused2_sweep_kernel<R4, NT><<<grid, NT, smem, stream>>>(
-        reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
-        first, keys);
+    if (coarse < 0)
+        fused2_sweep_kernel<R4, NT, false><<<grid, NT, smem, stream>>>(
+            reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
+            first, 0, keys);
+    else
+        fused2_sweep_kernel<R4, NT, true><<<grid, NT, smem, stream>>>(
+            reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
+            first, coarse, keys);
     return cudaGetLastError();
 }
 
@@ -409,16 +446,18 @@ inline cudaError_t plan_fused2(FusedPlan &plan, int L, int sm_count)
     }
 }
 
+// coarse < 0: the plain checkerboard sweep; coarse = 0 / 1: the double-checkerboard launch that
+// updates that coarse colour only (D14).
 inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
                                        uint64_t seed, int first, const FusedPlan &plan,
-                                       cudaStream_t stream)
+                                       cudaStream_t stream, int coarse = -1)
 {
     const SweepConsts keys = make_sweep_consts(seed, t, first);
     switch (L) {
-        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, keys, plan, stream);
-        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, keys, plan, stream);
-        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, keys, plan, stream);
-        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, keys, plan, stream);
+        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, coarse, keys, plan, stream);
+        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, coarse, keys, plan, stream);
+        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, coarse, keys, plan, stream);
+        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, coarse, keys, plan, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

@@ -351,11 +351,14 @@ def test_glauber_full_size_properties(B):
 # ------------------------------------------------------------------ f-2: double checkerboard
 @pytest.mark.parametrize("L,seed,variant,cps", [(64, 1, "auto", [1, 2, 6]), (128, 7, "auto", [1, 5]),
                                                 (256, 2, "auto", [2, 4]), (192, 8, "auto", [1, 3]),
-                                                (64, 3, "generic", [1, 4]), (512, 11, "auto", [1, 2])])
+                                                (64, 3, "generic", [1, 4]), (512, 11, "auto", [1, 2, 5]),
+                                                (512, 12, "generic", [1, 2]), (512, 13, "fused2", [3])])
 def test_double_checkerboard_against_oracle(B, orc, L, seed, variant, cps):
     sim = B.Ising3D(L, [seed], variant=VARIANTS(B)[variant])
     sim.set_cycle(B.CYCLE_DOUBLE_CB)
-    assert sim.variant_name in ("resident", "generic")
+    want = {"generic": "generic", "fused2": "fused2"}.get(variant, "fused2" if L in (512, 1024, 2048, 4096) else
+                                                          "resident" if L <= 256 and L != 192 else "generic")
+    assert sim.variant_name == want
     ref = orc.Oracle(L, seed)
     t = 0
     for cp in cps:
@@ -383,13 +386,42 @@ def test_double_checkerboard_batch_neel_and_errors(B, orc):
         ref.sweep_dcb(3, block=8)
         assert np.array_equal(st[i], ref.export_words())
     batch.free()
-    sim = B.Ising3D(512, [1])
+    sim = B.Ising3D(1024, [1])
     sim.set_cycle(B.CYCLE_DOUBLE_CB)
     with pytest.raises(B.Ising3DError):
-        sim.set_variant(B.VARIANT_FUSED2)
+        sim.set_variant(B.VARIANT_FUSED3)
+    with pytest.raises(B.Ising3DError):
+        sim.set_variant(B.VARIANT_ACTIVE)
     with pytest.raises(B.Ising3DError):
         sim.set_temperature(2.0)
     sim.free()
+
+
+@pytest.mark.parametrize("L,seed", [(1024, 21), (2048, 22)])
+def test_double_checkerboard_fused2_full_size(B, orc, L, seed):
+    """The masked fused2 launches (one per coarse colour) against the masked generic kernel word for
+    word, from the iid start and from a late-time-like state, and sampled sites against the oracle:
+    a site is recomputed through the four masked half-sweeps of one sweep by brute force."""
+    a = B.Ising3D(L, [seed])
+    a.set_cycle(B.CYCLE_DOUBLE_CB)
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_GENERIC)
+    b.set_cycle(B.CYCLE_DOUBLE_CB)
+    assert a.variant_name == "fused2" and b.variant_name == "generic"
+    a.sweep(3)
+    b.sweep(3)
+    assert np.array_equal(a.get_state(), b.get_state())
+    if L == 1024:
+        ref = orc.Oracle(L, seed)
+        ref.sweep_dcb(3, block=8)
+        assert np.array_equal(a.get_state(), ref.export_words())
+        words = inputs.coarse_words(L, 5, block=16)
+        a.set_state(words, 700)
+        ref.import_words(words, 700)
+        a.sweep(2)
+        ref.sweep_dcb(2, block=8)
+        assert np.array_equal(a.get_state(), ref.export_words())
+    a.free()
+    b.free()
 
 
 @pytest.mark.parametrize("L,seed,cps", [(64, 1, [1, 2, 6]), (128, 7, [1, 4]), (192, 8, [2]), (512, 11, [1, 2])])
