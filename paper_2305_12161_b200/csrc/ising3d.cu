@@ -666,11 +666,12 @@ int ising3d_set_temperature(ising3d_t *h, double T)
     h->temperature = T;
     if (T > 0.0) {
         // D13: thr[n] = floor(2^32 / (1 + exp((12 - 4n)/T))), fp64, n = antiparallel neighbours
+        for (int B = 0; B <= 32; ++B) h->glauber.lut[B] = 0u;
         for (int n = 0; n <= 6; ++n) {
             const double dE = 12.0 - 4.0 * (double)n;
             const double p = 1.0 / (1.0 + std::exp(dE / T));
             const uint64_t thr = (uint64_t)std::floor(p * 4294967296.0);
-            for (int B = 0; B <= 32; ++B) h->glauber.sel[B][n] = ((thr >> B) & 1u) ? 0xFFFFFFFFu : 0u;
+            for (int B = 0; B <= 32; ++B) h->glauber.lut[B] |= (uint32_t)((thr >> B) & 1u) << n;
         }
     }
     return ISING3D_OK;
