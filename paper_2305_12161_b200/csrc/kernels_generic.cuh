@@ -320,15 +320,26 @@ __device__ __forceinline__ uint4 class_select(const uint32_t lut, const uint4 c2
     return T;
 }
 
+// 32 x 32 -> 64 bit product as ONE IMAD.WIDE.U32 (written in PTX: inside the plane loop the C++
+// form picked up a dead add per product)
+__device__ __forceinline__ uint64_t mul_wide(uint32_t a, uint32_t b)
+{
+    uint64_t p;
+    asm("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(a), "r"(b));
+    return p;
+}
+
 __global__ void __launch_bounds__(256)
 halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restrict__ seeds, int L,
                          uint32_t t, int phase, int mixed, const __grid_constant__ GlauberTables tb)
 {
-    const int WPR = L >> 6;
-    const size_t WPC = (size_t)L * L * WPR;
-    const size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = g < WPC / 4;
-    const size_t gg = active ? g : 0;                           // idle lanes follow along (warp votes)
+    // all indices fit 32 bits: a colour has L^3/64 <= 2^30 words
+    const uint32_t WPR = (uint32_t)L >> 6, uL = (uint32_t)L;
+    const uint32_t WPCu = uL * uL * WPR;
+    const size_t WPC = WPCu;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = g < WPCu / 4;
+    const uint32_t gg = active ? g : 0;                         // idle lanes follow along (warp votes)
     const int rep = blockIdx.y;
     const uint64_t seed = seeds[rep];
     const int c = mixed ? phase ^ first_colour(seed, t) : phase;
@@ -338,25 +349,24 @@ halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
     const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
     uint32_t c0[4], c1[4], c2[4];                               // bit planes of n = antiparallel neighbours
     // rows of a multiple of four words (L % 256 == 0): the group lies in one row, one index split
-    const bool one_row = (WPR & 3) == 0;
-    const size_t row_g = (4 * gg) / WPR;
-    const int wi_g = (int)((4 * gg) % WPR), y_g = (int)(row_g % L), z_g = (int)(row_g / L);
+    const bool one_row = (WPR & 3u) == 0u;
+    const uint32_t row_g = (4u * gg) / WPR, wi_g = 4u * gg - row_g * WPR;
+    const uint32_t z_g = row_g / uL, y_g = row_g - z_g * uL;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const size_t w = 4 * gg + i;
-        int wi = wi_g + i, y = y_g, z = z_g;
-        size_t row = row_g;
+        const uint32_t w = 4u * gg + (uint32_t)i;
+        uint32_t wi = wi_g + (uint32_t)i, y = y_g, z = z_g, row = row_g;
         if (!one_row) {
-            wi = (int)(w % WPR);
             row = w / WPR;
-            y = (int)(row % L);
-            z = (int)(row / L);
+            wi = w - row * WPR;
+            z = row / uL;
+            y = row - z * uL;
         }
-        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
-        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const uint32_t yp = (y + 1 == uL) ? 0 : y + 1, ym = (y == 0) ? uL - 1 : y - 1;
+        const uint32_t zp = (z + 1 == uL) ? 0 : z + 1, zm = (z == 0) ? uL - 1 : z - 1;
         const uint32_t n_same = oth[w];
         uint32_t n_x;
-        if (((y + z + c) & 1) == 0) {
+        if (((y + z + (uint32_t)c) & 1u) == 0u) {
             const uint32_t prev = oth[row * WPR + (wi == 0 ? WPR - 1 : wi - 1)];
             n_x = (n_same << 1) | (prev >> 31);
         } else {
@@ -365,10 +375,10 @@ halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
         }
         // antiparallel indicators of the six neighbours
         const uint32_t d1 = s[i] ^ n_same, d2 = s[i] ^ n_x;
-        const uint32_t d3 = s[i] ^ oth[((size_t)z * L + yp) * WPR + wi];
-        const uint32_t d4 = s[i] ^ oth[((size_t)z * L + ym) * WPR + wi];
-        const uint32_t d5 = s[i] ^ oth[((size_t)zp * L + y) * WPR + wi];
-        const uint32_t d6 = s[i] ^ oth[((size_t)zm * L + y) * WPR + wi];
+        const uint32_t d3 = s[i] ^ oth[(z * uL + yp) * WPR + wi];
+        const uint32_t d4 = s[i] ^ oth[(z * uL + ym) * WPR + wi];
+        const uint32_t d5 = s[i] ^ oth[(zp * uL + y) * WPR + wi];
+        const uint32_t d6 = s[i] ^ oth[(zm * uL + y) * WPR + wi];
         const uint32_t sa = d1 ^ d2 ^ d3, ca = maj3(d1, d2, d3);
         const uint32_t sb = d4 ^ d5 ^ d6, cb = maj3(d4, d5, d6);
         const uint32_t k1 = sa & sb;
@@ -383,15 +393,15 @@ halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
         k0r[r] = (uint32_t)seed + (uint32_t)r * kPhiloxW0;
         k1r[r] = (uint32_t)(seed >> 32) + (uint32_t)r * kPhiloxW1;
     }
-    const uint32_t q = (uint32_t)gg;
-    const uint64_t q0 = (uint64_t)kPhiloxM0 * q;                            // round 0, p0
+    const uint32_t q = gg;
+    const uint64_t q0 = mul_wide(kPhiloxM0, q);                            // round 0, p0
     const uint32_t a0 = t ^ k0r[0];                                          // round-0 c0 (hi(M1*c) = 0)
     const uint32_t b0 = c ? kPhiloxM1 : 0u;                                  // round-0 c1 = lo(M1*c)
     const uint32_t x0 = (uint32_t)(q0 >> 32) ^ k1r[0];                       // round-0 c2 = x0 ^ tag
-    const uint64_t pa = (uint64_t)kPhiloxM0 * a0;                            // round 1, p0
+    const uint64_t pa = mul_wide(kPhiloxM0, a0);                            // round 1, p0
     const uint32_t r1c2 = (uint32_t)(pa >> 32) ^ (uint32_t)q0 ^ k1r[1];      // round-1 c2
     const uint32_t r1c3 = (uint32_t)pa;                                      // round-1 c3
-    const uint64_t pb = (uint64_t)kPhiloxM1 * r1c2;                          // round 2, p1
+    const uint64_t pb = mul_wide(kPhiloxM1, r1c2);                          // round 2, p1
     const uint4 C0 = make_uint4(c0[0], c0[1], c0[2], c0[3]), C1 = make_uint4(c1[0], c1[1], c1[2], c1[3]);
     const uint4 C2 = make_uint4(c2[0], c2[1], c2[2], c2[3]);
     uint4 lt = class_select(tb.lut[32], C2, C1, C0);            // the 2^32 bit: u has none
@@ -402,17 +412,17 @@ halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
         uint4 r;
         {
             const uint32_t tag = 4u + (uint32_t)j;
-            const uint64_t p1 = (uint64_t)kPhiloxM1 * (x0 ^ tag);            // round 1
+            const uint64_t p1 = mul_wide(kPhiloxM1, x0 ^ tag);            // round 1
             uint32_t v0 = (uint32_t)(p1 >> 32) ^ b0 ^ k0r[1], v1 = (uint32_t)p1;
-            uint64_t p0 = (uint64_t)kPhiloxM0 * v0;                          // round 2 (p1 = pb)
+            uint64_t p0 = mul_wide(kPhiloxM0, v0);                           // round 2 (p1 = pb)
             v0 = (uint32_t)(pb >> 32) ^ v1 ^ k0r[2];
             uint32_t v2 = (uint32_t)(p0 >> 32) ^ r1c3 ^ k1r[2];
             v1 = (uint32_t)pb;
             uint32_t v3 = (uint32_t)p0;
 #pragma unroll
             for (int rr = 3; rr < 10; ++rr) {
-                p0 = (uint64_t)kPhiloxM0 * v0;
-                const uint64_t p1r = (uint64_t)kPhiloxM1 * v2;
+                p0 = mul_wide(kPhiloxM0, v0);
+                const uint64_t p1r = mul_wide(kPhiloxM1, v2);
                 v0 = (uint32_t)(p1r >> 32) ^ v1 ^ k0r[rr];
                 v2 = (uint32_t)(p0 >> 32) ^ v3 ^ k1r[rr];
                 v1 = (uint32_t)p1r;

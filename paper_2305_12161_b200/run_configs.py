@@ -3,7 +3,8 @@
 the trajectory of the measured quantities and the throughput in site-updates/ns.
 
   python -m paper_2305_12161_b200.run_configs [--configs config1_L64,config5_L2048]
-         [--max-sweeps N] [--radial] [--out results.jsonl]
+         [--max-sweeps N] [--radial] [--variant V] [--cycle 01|mixed|dcb|dcb_mixed] [--temperature T]
+         [--out results.jsonl]
 
 Per workload: ising3d_init(_batch) from the workload's seeds, then for
 each measurement time T(n) (S12): ising3d_sweep(dt), ising3d_measure().  Reported:
@@ -34,7 +35,8 @@ def ell_from_C(C: np.ndarray, c: float = 0.5) -> float:
     return float("nan")
 
 
-def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto", radial: bool = False):
+def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto", radial: bool = False,
+                 cycle: str = "01", temperature: float = 0.0):
     import torch
     from . import binding
 
@@ -46,8 +48,13 @@ def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto",
         times.append(n_total)
     sim = binding.Ising3D(L, seeds, variant={"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
                                              "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2,
-                                             "fused3": binding.VARIANT_FUSED3,
+                                             "fused3": binding.VARIANT_FUSED3, "active": binding.VARIANT_ACTIVE,
                                              "resident": binding.VARIANT_RESIDENT}[variant])
+    if cycle != "01":
+        sim.set_cycle({"mixed": binding.CYCLE_MIXED, "dcb": binding.CYCLE_DOUBLE_CB,
+                       "dcb_mixed": binding.CYCLE_DOUBLE_CB_MIXED}[cycle])
+    if temperature > 0.0:
+        sim.set_temperature(temperature)
     N = L ** 3 * len(seeds)
     ev = lambda: torch.cuda.Event(enable_timing=True)
     t_sweeps = t_meas = t_rad = 0.0
@@ -72,6 +79,9 @@ def run_workload(name: str, max_sweeps: int | None, emit, variant: str = "auto",
                 "ell_nan": int(np.isnan(m["ell"]).sum())}
         if len(seeds) > 1:
             line["ell_of_mean_C"] = ell_from_C(m["C"].mean(axis=0))
+        line["kernel"] = sim.variant_name
+        if L >= 256 and (L & (L - 1)) == 0:
+            line["awake_group_fraction"] = sim.activity()[1]     # groups holding a Delta E <= 0 site
         if radial:      # the paper's estimator (eq. 7 + radial average), outside the timed totals
             e3, e4 = ev(), ev()
             e3.record()
@@ -102,8 +112,12 @@ def main(argv=None):
     ap.add_argument("--configs", default=",".join(inputs.WORKLOADS))
     ap.add_argument("--max-sweeps", type=int, default=None,
                     help="truncate each workload to this many sweeps (default: the full run)")
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "fused3", "resident"],
+    ap.add_argument("--variant", default="auto",
+                    choices=["auto", "generic", "fused", "fused2", "fused3", "resident", "active"],
                     help="sweep kernel (default: the library's choice)")
+    ap.add_argument("--cycle", default="01", choices=["01", "mixed", "dcb", "dcb_mixed"],
+                    help="update order (ising3d_set_cycle)")
+    ap.add_argument("--temperature", type=float, default=0.0, help="T > 0: Glauber dynamics, eq. (5)")
     ap.add_argument("--radial", action="store_true",
                     help="also call ising3d_measure_radial (FFT + radial average) at every checkpoint")
     ap.add_argument("--out", default=None, help="also append the JSON lines to this file")
@@ -120,7 +134,7 @@ def main(argv=None):
             fh.flush()
 
     for name in args.configs.split(","):
-        run_workload(name.strip(), args.max_sweeps, emit, args.variant, args.radial)
+        run_workload(name.strip(), args.max_sweeps, emit, args.variant, args.radial, args.cycle, args.temperature)
     return 0
 
 

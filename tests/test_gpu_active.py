@@ -209,3 +209,25 @@ def test_active_equals_fused2_at_full_size_late_time(B, orc):
     assert list(b.activity()[0][0]) == list(ref.activity())
     a.free()
     b.free()
+
+
+@pytest.mark.slow
+def test_auto_run_equals_fused2_run_config4(B):
+    """Config 4 (L = 1024, seed 3, 10^5 sweeps) run twice: under the AUTO policy (fused2, probes every
+    1024 sweeps, hand-over to the activity-driven kernel when under 7.5 % of the groups can change)
+    and on fused2 alone.  Every word of the final states and all counts must agree, and AUTO must
+    have handed over on the way."""
+    L, seed, n = 1024, 3, 100_000
+    a = B.Ising3D(L, [seed])
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED2)
+    a.sweep(n)
+    b.sweep(n)
+    assert a.variant_name == "active" and b.variant_name == "fused2"
+    assert 0.0 < a.last_activity < 0.075
+    ev = a.active_stats()[0]
+    assert ev[0] > 0 and ev[1] > 0
+    assert np.array_equal(a.get_state(), b.get_state())
+    ma, mb = a.measure(), b.measure()
+    assert int(ma["n_up"][0]) == int(mb["n_up"][0]) and np.array_equal(ma["antipar"], mb["antipar"])
+    a.free()
+    b.free()
