@@ -77,7 +77,7 @@ extern "C" {
                                        see ising3d_set_activity_policy), else generic           */
 #define ISING3D_VARIANT_GENERIC 1   /* two in-place half-sweep launches per sweep         */
 #define ISING3D_VARIANT_FUSED   2   /* one launch per sweep, black+white fused            */
-#define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in 512..4096); a batch
+#define ISING3D_VARIANT_FUSED2  3   /* fused, two rows per thread (L in {512,1024,1536,2048,4096}); a batch
                                        is swept replica by replica (n_rep launches per sweep) */
 #define ISING3D_VARIANT_RESIDENT 4  /* lattice resident in the shared memory of a thread-block
                                        cluster, all sweeps of a call in one launch (L in 64..256) */

@@ -733,7 +733,7 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (variant == ISING3D_VARIANT_FUSED && !h->fused_ok())
         return fail(ISING3D_EINVAL, "fused kernel needs L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED2 && !h->fused2_ok())
-        return fail(ISING3D_EINVAL, "fused2 kernel needs L in {512,1024,2048,4096}");
+        return fail(ISING3D_EINVAL, "fused2 kernel needs L in {512,1024,1536,2048,4096}");
     if (variant == ISING3D_VARIANT_FUSED3 && !h->fused3_ok())
         return fail(ISING3D_EINVAL, "fused3 kernel needs L in {1024,2048}");
     if (variant == ISING3D_VARIANT_RESIDENT && !h->resident_ok())

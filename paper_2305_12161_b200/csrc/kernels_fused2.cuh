@@ -231,6 +231,8 @@ __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, c
     }
 }
 
+__host__ __device__ constexpr int f2_row_lanes(int r4) { return r4 <= 1 ? 1 : r4 <= 2 ? 2 : r4 <= 4 ? 4 : r4 <= 8 ? 8 : r4 <= 16 ? 16 : 32; }
+
 // Grid: blockIdx.x = y tile (RPT stored rows each, RPT even), blockIdx.y = z chunk.
 // Chunk boundaries are odd planes, so the first marched plane z0 = zs-3 is even and the
 // in-row direction of the even tile row at step k is k & 1.
@@ -242,10 +244,13 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
                     const int RPT, const int nzc, const int first, const int coarse,
                     const __grid_constant__ SweepConsts keys)
 {
-    constexpr int TY = 2 * NT / R4;    // rows in the tile (incl. 2+2 halo rows)
+    // R4 = groups per row (L / 256); a row takes RL = the next power of two lanes of a warp (L = 1536:
+    // 6 groups on 8 lanes; the two spare lanes of a row repeat its last group and store nothing)
+    constexpr int RL = f2_row_lanes(R4);
+    constexpr int TY = 2 * NT / RL;    // rows in the tile (incl. 2+2 halo rows)
     constexpr int PLANE = TY * R4;     // uint4 per plane tile
     constexpr int S = kF2Stages, D = S - 1;
-    static_assert(R4 <= 32 && (32 % R4) == 0, "a row must fit a warp");
+    static_assert(RL <= 32, "a row must fit a warp");
 
     extern __shared__ __align__(128) uint4 smem[];
     uint4 *Wst = smem;                     // [S][PLANE]  W_old planes
@@ -254,7 +259,9 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     uint64_t *bars = reinterpret_cast<uint64_t *>(nb + 2 * PLANE);
 
     const int tid = threadIdx.x, lane = tid & 31;
-    const int x4 = tid & (R4 - 1), p = tid / R4;     // group column, row pair
+    const int x4l = tid & (RL - 1), p = tid / RL;    // lane inside the row, row pair
+    const int x4 = (R4 != RL && x4l >= R4) ? R4 - 1 : x4l;   // group column
+    const bool spare = R4 != RL && x4l >= R4;
     const int ry = 2 * p;                            // even tile row of this thread
     const int jt = blockIdx.x, zc = blockIdx.y;
     // chunk borders have the parity of 1-first, so that (z0 + first) is even for z0 = zs-3 and
@@ -283,12 +290,12 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     c.si0 = ry * R4 + x4;
     c.si_ym = ry > 0 ? c.si0 - R4 : c.si0;
     c.si_yp = ry + 2 < TY ? c.si0 + 2 * R4 : c.si0;
-    c.lane_prev = (lane & ~(R4 - 1)) | ((lane - 1) & (R4 - 1));
-    c.lane_next = (lane & ~(R4 - 1)) | ((lane + 1) & (R4 - 1));
+    c.lane_prev = (lane & ~(RL - 1)) | (x4 == 0 ? R4 - 1 : x4 - 1);
+    c.lane_next = (lane & ~(RL - 1)) | (x4 == R4 - 1 ? 0 : x4 + 1);
     c.qrow = (uint32_t)(y * R4 + x4);
     c.qplane = (uint32_t)(L * R4);
-    c.ok0 = (ry >= 2) && (ry - 2 < RPT) && (jt * RPT + ry - 2 < L);
-    c.ok1 = (ry + 1 - 2 < RPT) && (ry + 1 < TY - 2) && (jt * RPT + ry + 1 - 2 < L) && (ry >= 2);
+    c.ok0 = !spare && (ry >= 2) && (ry - 2 < RPT) && (jt * RPT + ry - 2 < L);
+    c.ok1 = !spare && (ry + 1 - 2 < RPT) && (ry + 1 < TY - 2) && (jt * RPT + ry + 1 - 2 < L) && (ry >= 2);
     c.nz = nz;
 
     if (tid == 0) {
@@ -380,12 +387,12 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
 // ---------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------
-inline bool fused2_supported(int L) { return L == 512 || L == 1024 || L == 2048 || L == 4096; }
+inline bool fused2_supported(int L) { return L == 512 || L == 1024 || L == 1536 || L == 2048 || L == 4096; }
 
 template <int R4, int NT>
 inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
 {
-    constexpr int TY = 2 * NT / R4;
+    constexpr int TY = 2 * NT / f2_row_lanes(R4);
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
     cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, false>,
@@ -420,7 +427,7 @@ template <int R4, int NT>
 inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first, int coarse,
                                    const SweepConsts &keys, const FusedPlan &plan, cudaStream_t stream)
 {
-    constexpr int TY = 2 * NT / R4;
+    constexpr int TY = 2 * NT / f2_row_lanes(R4);
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
     dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
@@ -440,6 +447,7 @@ inline cudaError_t plan_fused2(FusedPlan &plan, int L, int sm_count)
     switch (L) {
         case 512:  return plan_fused2_t<2, 128>(plan, L, sm_count);
         case 1024: return plan_fused2_t<4, 256>(plan, L, sm_count);
+        case 1536: return plan_fused2_t<6, 256>(plan, L, sm_count);
         case 2048: return plan_fused2_t<8, 256>(plan, L, sm_count);
         case 4096: return plan_fused2_t<16, 256>(plan, L, sm_count);
         default:   return cudaErrorInvalidValue;
@@ -456,6 +464,7 @@ inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L
     switch (L) {
         case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, coarse, keys, plan, stream);
         case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, coarse, keys, plan, stream);
+        case 1536: return launch_fused2_t<6, 256>(src, dst, L, first, coarse, keys, plan, stream);
         case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, coarse, keys, plan, stream);
         case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, coarse, keys, plan, stream);
         default:   return cudaErrorInvalidValue;
