@@ -390,6 +390,7 @@ def run_ours(args):
     roofline = {
         "bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
         "frac": achieved / peak, "traffic": traffic,
+        "frac_algorithmic_3N8": achieved / peak,      # the same number under the name of its byte model
         # what binds the kernel is the issue rate of its integer instructions, not HBM:
         "binding_limit": "issue",
         "issue_frac": sweep_rate / alu_bound,

@@ -348,43 +348,62 @@ halfsweep_glauber_kernel(uint32_t *__restrict__ state, const uint64_t *__restric
     const uint4 sv = reinterpret_cast<const uint4 *>(own)[gg];
     const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
     uint32_t c0[4], c1[4], c2[4];                               // bit planes of n = antiparallel neighbours
-    // rows of a multiple of four words (L % 256 == 0): the group lies in one row, one index split
-    const bool one_row = (WPR & 3u) == 0u;
-    const uint32_t row_g = (4u * gg) / WPR, wi_g = 4u * gg - row_g * WPR;
-    const uint32_t z_g = row_g / uL, y_g = row_g - z_g * uL;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const uint32_t w = 4u * gg + (uint32_t)i;
-        uint32_t wi = wi_g + (uint32_t)i, y = y_g, z = z_g, row = row_g;
-        if (!one_row) {
-            row = w / WPR;
-            wi = w - row * WPR;
-            z = row / uL;
-            y = row - z * uL;
-        }
-        const uint32_t yp = (y + 1 == uL) ? 0 : y + 1, ym = (y == 0) ? uL - 1 : y - 1;
-        const uint32_t zp = (z + 1 == uL) ? 0 : z + 1, zm = (z == 0) ? uL - 1 : z - 1;
-        const uint32_t n_same = oth[w];
-        uint32_t n_x;
-        if (((y + z + (uint32_t)c) & 1u) == 0u) {
-            const uint32_t prev = oth[row * WPR + (wi == 0 ? WPR - 1 : wi - 1)];
-            n_x = (n_same << 1) | (prev >> 31);
-        } else {
-            const uint32_t next = oth[row * WPR + (wi == WPR - 1 ? 0 : wi + 1)];
-            n_x = (n_same >> 1) | (next << 31);
-        }
-        // antiparallel indicators of the six neighbours
-        const uint32_t d1 = s[i] ^ n_same, d2 = s[i] ^ n_x;
-        const uint32_t d3 = s[i] ^ oth[(z * uL + yp) * WPR + wi];
-        const uint32_t d4 = s[i] ^ oth[(z * uL + ym) * WPR + wi];
-        const uint32_t d5 = s[i] ^ oth[(zp * uL + y) * WPR + wi];
-        const uint32_t d6 = s[i] ^ oth[(zm * uL + y) * WPR + wi];
+    // n = antiparallel neighbours of the 32 sites of word i, as three bit planes (two 3:2 compressors)
+    auto count = [&](int i, uint32_t n_same, uint32_t n_x, uint32_t n_yp, uint32_t n_ym, uint32_t n_zp, uint32_t n_zm) {
+        const uint32_t d1 = s[i] ^ n_same, d2 = s[i] ^ n_x, d3 = s[i] ^ n_yp;
+        const uint32_t d4 = s[i] ^ n_ym, d5 = s[i] ^ n_zp, d6 = s[i] ^ n_zm;
         const uint32_t sa = d1 ^ d2 ^ d3, ca = maj3(d1, d2, d3);
         const uint32_t sb = d4 ^ d5 ^ d6, cb = maj3(d4, d5, d6);
         const uint32_t k1 = sa & sb;
         c0[i] = sa ^ sb;
         c1[i] = ca ^ cb ^ k1;
         c2[i] = maj3(ca, cb, k1);
+    };
+    if ((WPR & 3u) == 0u) {
+        // rows of a multiple of four words (L % 256 == 0): the group lies in one row, so the six
+        // neighbour words of all four words come as five 128-bit loads and one edge word (D4)
+        const uint32_t R4 = WPR >> 2, row = gg / R4, x4 = gg - row * R4;
+        const uint32_t z = row / uL, y = row - z * uL;
+        const uint32_t yp = (y + 1 == uL) ? 0 : y + 1, ym = (y == 0) ? uL - 1 : y - 1;
+        const uint32_t zp = (z + 1 == uL) ? 0 : z + 1, zm = (z == 0) ? uL - 1 : z - 1;
+        const uint4 *oth4 = reinterpret_cast<const uint4 *>(oth);
+        const uint4 a = oth4[gg];
+        const uint4 vyp = oth4[(z * uL + yp) * R4 + x4], vym = oth4[(z * uL + ym) * R4 + x4];
+        const uint4 vzp = oth4[(zp * uL + y) * R4 + x4], vzm = oth4[(zm * uL + y) * R4 + x4];
+        uint4 x;
+        if (((y + z + (uint32_t)c) & 1u) == 0u) {           // neighbour k-1: bit j <- bit j-1
+            const uint32_t edge = oth[4u * (row * R4 + (x4 == 0 ? R4 - 1 : x4 - 1)) + 3u];
+            x = make_uint4((a.x << 1) | (edge >> 31), (a.y << 1) | (a.x >> 31), (a.z << 1) | (a.y >> 31),
+                           (a.w << 1) | (a.z >> 31));
+        } else {                                            // neighbour k+1: bit j <- bit j+1
+            const uint32_t edge = oth[4u * (row * R4 + (x4 == R4 - 1 ? 0 : x4 + 1))];
+            x = make_uint4((a.x >> 1) | (a.y << 31), (a.y >> 1) | (a.z << 31), (a.z >> 1) | (a.w << 31),
+                           (a.w >> 1) | (edge << 31));
+        }
+        count(0, a.x, x.x, vyp.x, vym.x, vzp.x, vzm.x);
+        count(1, a.y, x.y, vyp.y, vym.y, vzp.y, vzm.y);
+        count(2, a.z, x.z, vyp.z, vym.z, vzp.z, vzm.z);
+        count(3, a.w, x.w, vyp.w, vym.w, vzp.w, vzm.w);
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t w = 4u * gg + (uint32_t)i;
+            const uint32_t row = w / WPR, wi = w - row * WPR;
+            const uint32_t z = row / uL, y = row - z * uL;
+            const uint32_t yp = (y + 1 == uL) ? 0 : y + 1, ym = (y == 0) ? uL - 1 : y - 1;
+            const uint32_t zp = (z + 1 == uL) ? 0 : z + 1, zm = (z == 0) ? uL - 1 : z - 1;
+            const uint32_t n_same = oth[w];
+            uint32_t n_x;
+            if (((y + z + (uint32_t)c) & 1u) == 0u) {
+                const uint32_t prev = oth[row * WPR + (wi == 0 ? WPR - 1 : wi - 1)];
+                n_x = (n_same << 1) | (prev >> 31);
+            } else {
+                const uint32_t next = oth[row * WPR + (wi == WPR - 1 ? 0 : wi + 1)];
+                n_x = (n_same >> 1) | (next << 31);
+            }
+            count(i, n_same, n_x, oth[(z * uL + yp) * WPR + wi], oth[(z * uL + ym) * WPR + wi],
+                  oth[(zp * uL + y) * WPR + wi], oth[(zm * uL + y) * WPR + wi]);
+        }
     }
     // Philox4x32-10 of counter (q, t, c, 4 + j), key = seed: the plane-independent parts
     uint32_t k0r[10], k1r[10];
