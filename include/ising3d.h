@@ -307,6 +307,12 @@ typedef struct {
 } ising3d_radial_t;
 int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out);
 
+/* Exactness margin of the last ising3d_measure_radial call (D12): the largest distance of an
+ * inverse-transform value / N from the integer it was rounded to, over all displacements and
+ * replicas; P(d) is exact as long as this stays below 1/2 (it is of order 1e-4 at L = 2048).
+ * HOST pointer; -1 before the first call. */
+int ising3d_radial_rounding(const ising3d_t *h, double *max_distance);
+
 /* Give back the device memory and cuFFT plans ising3d_measure_radial keeps between calls
  * (8 bytes per site + work area: 128 GiB at L = 2048).  The next call re-creates them. */
 int ising3d_release_radial(ising3d_t *h);

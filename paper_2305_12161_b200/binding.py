@@ -27,7 +27,7 @@ EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
     "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_set_temperature", "ising3d_init_menger", "ising3d_set_measure_variant",
     "ising3d_measure_variant_name",
-    "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
+    "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_radial_rounding", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
     "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size",
     "ising3d_set_cluster_size", "ising3d_activity", "ising3d_active_stats", "ising3d_set_activity_policy", "ising3d_sync",
@@ -86,6 +86,7 @@ def load():
         "ising3d_sweep": (C.c_int, [vp, u64]),
         "ising3d_measure": (C.c_int, [vp, C.POINTER(MeasT)]),
         "ising3d_measure_radial": (C.c_int, [vp, C.POINTER(RadialT)]),
+        "ising3d_radial_rounding": (C.c_int, [vp, C.POINTER(C.c_double)]),
         "ising3d_release_radial": (C.c_int, [vp]),
         "ising3d_get_state": (C.c_int, [vp, vp, C.c_size_t, u64p]),
         "ising3d_set_state": (C.c_int, [vp, vp, C.c_size_t, u64]),
@@ -285,6 +286,13 @@ class Ising3D:
                     float(c_intercept))
         _check(self._l.ising3d_measure_radial(self._h, C.byref(m)))
         return {"sweep": int(m.sweep), "corr_sum": corr, "shell": shell, "C_rad": Cr, "S_rad": Sr, "ell": ell}
+
+    @property
+    def radial_rounding(self) -> float:
+        """max |v/N - round(v/N)| of the last measure_radial call (exactness margin, D12)."""
+        d = C.c_double()
+        _check(self._l.ising3d_radial_rounding(self._h, C.byref(d)))
+        return float(d.value)
 
     def release_radial(self):
         _check(self._l.ising3d_release_radial(self._h))

@@ -70,7 +70,8 @@ struct ising3d {
     // FFT estimator (ising3d_measure_radial): created on first use, library-owned
     double *fft_buf = nullptr;                 // [L][L][L+2] in-place real / half-complex field
     void *fft_work = nullptr;                  // cuFFT work area shared by both plans
-    unsigned long long *d_rad = nullptr;       // [2][L/2+1] P sums, shell counts; then [L/2+1] doubles
+    unsigned long long *d_rad = nullptr;       // [2][L/2+1] P sums, shell counts; [L/2+1] doubles; max rounding distance
+    double radial_rounding = -1.0;             // max |v/N - llrint(v/N)| of the last measure_radial call
     cufftHandle plan_fwd = 0, plan_inv = 0;
     bool fft_ready = false;
     uint64_t launches = 0;
@@ -531,7 +532,7 @@ int fft_setup(ising3d *h)
     };
     size_t ws_f = 0, ws_i = 0;
     if (cudaMalloc(&h->fft_buf, buf_bytes) != cudaSuccess ||
-        cudaMalloc(&h->d_rad, (size_t)3 * H * 8) != cudaSuccess) {
+        cudaMalloc(&h->d_rad, ((size_t)3 * H + 1) * 8) != cudaSuccess) {
         cleanup();
         return fail(ISING3D_ENOMEM, "radial estimator: cannot allocate the 8 bytes/site FFT field");
     }
@@ -909,14 +910,15 @@ int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out)
     if (cufftSetStream(h->plan_fwd, h->stream) != CUFFT_SUCCESS ||
         cufftSetStream(h->plan_inv, h->stream) != CUFFT_SUCCESS)
         return fail(ISING3D_ECUDA, "cufftSetStream failed");
-    std::vector<unsigned long long> host((size_t)3 * H);
+    std::vector<unsigned long long> host((size_t)3 * H + 1);
     const int grid = h->sm_count * 8;
+    h->radial_rounding = 0.0;
     out->sweep = h->sweep;
     for (int rep = 0; rep < h->n_rep; ++rep) {
         const uint32_t *st = h->state[h->cur] + (size_t)rep * h->words_per_replica();
         unsigned long long *d_cnt = h->d_counts + (size_t)rep * cpr;
         CUDA_TRY(cudaMemsetAsync(d_cnt, 0, 8, h->stream));
-        CUDA_TRY(cudaMemsetAsync(h->d_rad, 0, (size_t)3 * H * 8, h->stream));
+        CUDA_TRY(cudaMemsetAsync(h->d_rad, 0, ((size_t)3 * H + 1) * 8, h->stream));
         ising::count_up_kernel<<<dim3((unsigned)grid, 1), 256, 0, h->stream>>>(st, d_cnt, h->words_per_replica(), cpr);
         ising::unpack_real_kernel<<<grid, 256, 0, h->stream>>>(st, h->fft_buf, L);
         if (cufftExecD2Z(h->plan_fwd, h->fft_buf, reinterpret_cast<cufftDoubleComplex *>(h->fft_buf)) != CUFFT_SUCCESS)
@@ -925,13 +927,19 @@ int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out)
             reinterpret_cast<double2 *>(h->fft_buf), reinterpret_cast<double *>(h->d_rad + 2 * H), L);
         if (cufftExecZ2D(h->plan_inv, reinterpret_cast<cufftDoubleComplex *>(h->fft_buf), h->fft_buf) != CUFFT_SUCCESS)
             return fail(ISING3D_ECUDA, "cufftExecZ2D failed");
-        ising::radial_kernel<<<grid, 256, (size_t)2 * H * 8, h->stream>>>(h->fft_buf, h->d_rad, h->d_rad + H, L);
+        ising::radial_kernel<<<grid, 256, (size_t)2 * H * 8, h->stream>>>(h->fft_buf, h->d_rad, h->d_rad + H,
+                                                                          h->d_rad + 3 * H, L);
         h->launches += 4;
         CUDA_TRY(cudaGetLastError());
         unsigned long long n_up = 0;
         CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_rad, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
         CUDA_TRY(cudaMemcpyAsync(&n_up, d_cnt, 8, cudaMemcpyDeviceToHost, h->stream));
         CUDA_TRY(cudaStreamSynchronize(h->stream));
+        {
+            double dev;
+            std::memcpy(&dev, &host[3 * H], 8);
+            h->radial_rounding = std::max(h->radial_rounding, dev);
+        }
         // D12 / D9 post-processing in fp64, this order
         const double m = (double)(2 * (int64_t)n_up - (int64_t)N) / N;
         double *C = out->C_rad + (size_t)rep * H;
@@ -955,6 +963,13 @@ int ising3d_measure_radial(ising3d_t *h, ising3d_radial_t *out)
                 }
         }
     }
+    return ISING3D_OK;
+}
+
+int ising3d_radial_rounding(const ising3d_t *h, double *max_distance)
+{
+    if (!h || !max_distance) return fail(ISING3D_EINVAL, "null pointer");
+    *max_distance = h->radial_rounding;
     return ISING3D_OK;
 }
 

@@ -84,7 +84,7 @@ power_kernel(double2 *__restrict__ buf, double *__restrict__ s_sum, const int L)
 // radial sums of the integer correlation matrix P(d) = llrint(buf[d] / N) and the bin populations
 __global__ void __launch_bounds__(256)
 radial_kernel(const double *__restrict__ buf, unsigned long long *__restrict__ p_sum,
-              unsigned long long *__restrict__ shell, const int L)
+              unsigned long long *__restrict__ shell, unsigned long long *__restrict__ max_dev_bits, const int L)
 {
     extern __shared__ unsigned long long rd_smem[];          // [2][L/2 + 1]
     const int H = L / 2 + 1, LP = L + 2;
@@ -92,6 +92,7 @@ radial_kernel(const double *__restrict__ buf, unsigned long long *__restrict__ p
     __syncthreads();
     const double inv_n = 1.0 / ((double)L * (double)L * (double)L);
     const size_t n = (size_t)L * L * L;
+    double dev = 0.0;                                        // exactness margin of D12: max |v/N - P|
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (size_t)gridDim.x * blockDim.x) {
         const int dx = (int)(i % L);
@@ -99,7 +100,9 @@ radial_kernel(const double *__restrict__ buf, unsigned long long *__restrict__ p
         const int dy = (int)(r % L), dz = (int)(r / L);
         const int b = radial_bin_dev(L, dx, dy, dz);
         if (b < H) {
-            const long long P = llrint(buf[r * LP + dx] * inv_n);
+            const double v = buf[r * LP + dx] * inv_n;
+            const long long P = llrint(v);
+            dev = fmax(dev, fabs(v - (double)P));
             atomicAdd(&rd_smem[b], (unsigned long long)P);   // two's complement: sums of signed values
             atomicAdd(&rd_smem[H + b], 1ull);
         }
@@ -109,6 +112,9 @@ radial_kernel(const double *__restrict__ buf, unsigned long long *__restrict__ p
         if (rd_smem[b]) atomicAdd(&p_sum[b], rd_smem[b]);
         if (rd_smem[H + b]) atomicAdd(&shell[b], rd_smem[H + b]);
     }
+    for (int o = 16; o; o >>= 1) dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
+    // non-negative doubles order like their bit patterns
+    if ((threadIdx.x & 31) == 0 && dev > 0.0) atomicMax(max_dev_bits, (unsigned long long)__double_as_longlong(dev));
 }
 
 }  // namespace ising

@@ -227,13 +227,16 @@ def _check_radial(got, want, rep=0):
         assert abs(got["ell"][rep] - want["ell"]) <= 1e-12 * abs(want["ell"])
 
 
-@pytest.mark.parametrize("L,seed,sweeps", [(64, 1, 0), (64, 1, 12), (128, 7, 5), (192, 8, 3), (256, 2, 20)])
+@pytest.mark.parametrize("L,seed,sweeps", [(64, 1, 0), (64, 1, 12), (128, 7, 5), (192, 8, 3), (256, 2, 20),
+                                           (512, 11, 6)])
 def test_radial_estimator_against_oracle(B, orc, L, seed, sweeps):
     sim = B.Ising3D(L, [seed])
     ref = orc.Oracle(L, seed)
+    assert sim.radial_rounding == -1.0
     sim.sweep(sweeps)
     ref.sweep(sweeps)
     _check_radial(sim.measure_radial(), ref.measure_radial())
+    assert 0.0 <= sim.radial_rounding < 1e-3            # exactness margin of the llrint (D12)
     # measuring does not disturb the state or the other measurement
     assert np.array_equal(sim.get_state(), ref.export_words())
     check_measure(sim.measure(), ref.measure_full())
@@ -282,6 +285,25 @@ def test_radial_estimator_large_identities(B):
     assert torch.cuda.mem_get_info()[0] > free0 + 8 * 2 ** 30
     r2 = sim.measure_radial()                          # and are re-created on demand
     assert np.array_equal(r2["corr_sum"], r["corr_sum"])
+    assert 0.0 < sim.radial_rounding < 1e-2
+    print("radial rounding margin at L=%d: %.3e" % (L, sim.radial_rounding))
+    sim.free()
+
+
+@pytest.mark.slow
+def test_radial_estimator_L2048_rounding_margin(B):
+    """D12 claims the inverse transform of +-1 data at L = 2048 is within 1e-3 of an integer multiple of
+    N, so llrint recovers P(d) exactly: measured here (64 GiB field + cuFFT work area), together with
+    the identities that hold at any size."""
+    L = 2048
+    sim = B.Ising3D(L, [4])
+    sim.sweep(20)
+    r = sim.measure_radial()
+    N = L ** 3
+    assert int(r["corr_sum"][0][0]) == N and int(r["shell"][0]) == 1 and int(r["shell"][1]) == 18
+    dev = sim.radial_rounding
+    print("radial rounding margin at L=2048: %.3e" % dev)
+    assert 0.0 < dev < 1e-2
     sim.free()
 
 
