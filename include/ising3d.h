@@ -191,9 +191,10 @@ int ising3d_init_menger(ising3d_t *h, int k);
  * dark then light sites inside it) and generic kernels.  Its mixed cycle (Table I;
  * reading D15): the coarse colour updated first in sweep t is the D10 bit; block
  * Bi = (bz*nB + by)*nB + bx (nB = L/8) updates first the fine colour given by bit (Bi & 127) of
- * Philox(key = seed, counter = (Bi >> 7, t, 0, 36)), then the other; generic kernel only (the
- * block bits of a sweep are drawn into the handle's idle state buffer).  Takes effect from the
- * next sweep.
+ * Philox(key = seed, counter = (Bi >> 7, t, 0, 36)), then the other; fused2 (L in 512..4096: the
+ * block bits of a sweep are drawn into a bit array, then per coarse colour one masked launch for
+ * the blocks that drew "dark first" and one for those that drew "light first") and generic
+ * kernels.  Takes effect from the next sweep.
  * EINVAL for an unknown value, with ISING3D_VARIANT_FUSED (01 cycle only), for the double
  * checkerboard with ISING3D_VARIANT_FUSED3 or _ACTIVE, or at T > 0 for anything but the 01 cycle.
  */

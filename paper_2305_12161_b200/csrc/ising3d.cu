@@ -86,6 +86,7 @@ struct ising3d {
     uint32_t *d_awake = nullptr;               // [n_rep][2][G/32]; valid only while flags_valid
     unsigned long long *d_act = nullptr;       // [n_rep][4]: flag counts of colour 0, 1; groups evaluated, changed
     unsigned int *d_tickets = nullptr;         // work-item counter of active_halfsweep_kernel (never reset)
+    uint32_t *d_ff = nullptr;                  // [n_rep][(L/8)^3/32] block-order bits of the current sweep (D15, fused2)
     ising::ActivePlan plan_act;
     bool flags_valid = false;                  // the flags describe state[cur] (set by activity_flags, kept by active sweeps)
     bool active_mode = false;                  // AUTO: the activity-driven kernel is the one being dispatched
@@ -123,7 +124,6 @@ struct ising3d {
     bool use_fused3() const { return variant == ISING3D_VARIANT_FUSED3 && cycle == ISING3D_CYCLE_01; }
     bool use_fused2() const
     {
-        if (cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED) return false;   // per-block orders: generic kernel
         return variant == ISING3D_VARIANT_FUSED2 || variant == ISING3D_VARIANT_FUSED3 ||
                (variant == ISING3D_VARIANT_AUTO && fused2_ok());
     }
@@ -156,7 +156,7 @@ struct ising3d {
 namespace {
 
 struct Layout {
-    size_t state, seeds, counts, gsum, queue, awake, act, total;
+    size_t state, seeds, counts, gsum, queue, awake, act, ff, total;
 };
 
 Layout make_layout(int L, int n_rep)
@@ -170,7 +170,8 @@ Layout make_layout(int L, int n_rep)
     const bool act = ising::active_supported(L);
     l.awake = act ? align_up((size_t)n_rep * 2 * ((size_t)L * L * (L >> 8) / 8), 256) : 0;
     l.act = act ? align_up((size_t)n_rep * 4 * 8, 256) + 256 : 0;        // + the ticket counter
-    l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue + l.awake + l.act;
+    l.ff = ising::fused2_supported(L) ? align_up((size_t)n_rep * ((size_t)(L / 8) * (L / 8) * (L / 8) / 8), 256) : 0;
+    l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue + l.awake + l.act + l.ff;
     return l;
 }
 
@@ -233,6 +234,9 @@ int create(ising3d_t **out, int L, int n_rep, const uint64_t *seeds, void *dev_b
                                               lay.queue + lay.awake);
             h->d_tickets = (unsigned int *)((char *)h->d_act + lay.act - 256);
         }
+        if (lay.ff)
+            h->d_ff = (uint32_t *)(p + 2 * lay.state + lay.seeds + lay.counts + lay.gsum + lay.queue + lay.awake +
+                                   lay.act);
         int dev = 0;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
             (e = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev)) !=
@@ -356,8 +360,15 @@ int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
         h->cur = 1 - h->cur;
         h->launches += h->n_rep;
     }
+    const bool dcbm = gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED;
+    const int nB = h->L / 8, ff_words = nB * nB * nB / 32;
     for (; i < n; ++i) {
         const uint32_t t = (uint32_t)(h->sweep + i0 + i);
+        if (dcbm) {     // D15: this sweep's fine order of every block, all replicas
+            ising::block_order_kernel<<<dim3((unsigned)((ff_words + 255) / 256), (unsigned)h->n_rep), 256, 0,
+                                        h->stream>>>(h->d_ff, (size_t)ff_words, h->d_seeds, ff_words, t);
+            h->launches += 1;
+        }
         for (int rep = 0; rep < h->n_rep; ++rep) {
             const uint64_t seed = h->seeds[rep];
             const uint32_t *src = h->state[h->cur] + rep * wpr;
@@ -365,7 +376,20 @@ int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
             // mixed cycle (D10): the launch layer draws this sweep's first colour on the host
             const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
             cudaError_t e;
-            if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
+            if (dcbm) {
+                // D15: the coarse colours in the drawn order; for each, the blocks that drew "dark first"
+                // and the blocks that drew "light first" in one masked launch each (blocks of one coarse
+                // colour do not touch): src -> dst -> src -> dst -> src
+                const uint32_t *ffr = h->d_ff + (size_t)rep * ff_words;
+                uint32_t *a = const_cast<uint32_t *>(src), *b = dst;
+                e = cudaSuccess;
+                for (int k = 0; k < 2 && e == cudaSuccess; ++k)
+                    for (int f = 0; f < 2 && e == cudaSuccess; ++f) {
+                        e = ising::launch_fused2_sweep(a, b, h->L, t, seed, f, h->plan_f2, h->stream,
+                                                       k ^ ising::first_colour(seed, t), ffr);
+                        std::swap(a, b);
+                    }
+            } else if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
                 // D14: the red blocks (dark, then light sites), then the blue blocks: two masked
                 // launches, src -> dst -> src
                 e = ising::launch_fused2_sweep(src, dst, h->L, t, seed, 0, h->plan_f2, h->stream, 0);
@@ -380,7 +404,9 @@ int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
             if (e != cudaSuccess)
                 return fail(ISING3D_ECUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
         }
-        if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
+        if (dcbm) {
+            h->launches += 4 * (uint64_t)h->n_rep;         // back in state[cur]
+        } else if (gen2 && h->cycle == ISING3D_CYCLE_DOUBLE_CB) {
             h->launches += 2 * (uint64_t)h->n_rep;         // back in state[cur]
         } else {
             h->cur = 1 - h->cur;
@@ -684,8 +710,8 @@ int ising3d_set_cycle(ising3d_t *h, int cycle)
     if (cycle < ISING3D_CYCLE_01 || cycle > ISING3D_CYCLE_DOUBLE_CB_MIXED)
         return fail(ISING3D_EINVAL, "unknown cycle");
     if (cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && h->variant != ISING3D_VARIANT_AUTO &&
-        h->variant != ISING3D_VARIANT_GENERIC)
-        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
+        h->variant != ISING3D_VARIANT_GENERIC && h->variant != ISING3D_VARIANT_FUSED2)
+        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the fused2 and generic kernels");
     if (cycle != ISING3D_CYCLE_01 && h->temperature > 0.0)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
     if (cycle != ISING3D_CYCLE_01 && h->variant == ISING3D_VARIANT_FUSED)
@@ -725,9 +751,9 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (variant == ISING3D_VARIANT_ACTIVE && h->cycle >= ISING3D_CYCLE_DOUBLE_CB)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
     if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
-        variant != ISING3D_VARIANT_GENERIC)
-        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the generic kernel");
-    if (variant == ISING3D_VARIANT_FUSED3 && h->cycle == ISING3D_CYCLE_DOUBLE_CB)
+        variant != ISING3D_VARIANT_GENERIC && variant != ISING3D_VARIANT_FUSED2)
+        return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the fused2 and generic kernels");
+    if (variant == ISING3D_VARIANT_FUSED3 && h->cycle >= ISING3D_CYCLE_DOUBLE_CB)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
     if (variant == ISING3D_VARIANT_FUSED && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "the first-generation fused kernel runs the 01 cycle only");

@@ -157,20 +157,33 @@ struct F2Ctx {
 // U = position of the step in the 6-step unrolled march (k = 6 lap + U).  With a ring of 3 or 6 stages
 // the stage of the step, and with it every shared-memory address, is base + immediate; the mbarrier
 // parity is U/3 (S = 3) or the parity of the lap (S = 6).  The exchange plane index is U & 1.
-// DCB (double checkerboard, Supp. I.A PAPER.md:223-240, D14): only the sites of one coarse colour are
-// updated in this launch; mB / mW are the bit masks of those sites in the words of this thread's two
-// rows (same block row) at the black plane z and at the white plane z-1; the other sites keep their
-// old value (they are the frozen halo of the blocks being updated).
-__device__ __forceinline__ uint4 keep_unmasked(const uint4 upd, const uint4 old, const uint32_t m)
+// DCB (double checkerboard, Supp. I.A PAPER.md:223-240): only some blocks are updated in this launch;
+// mB / mW are the bit masks of their sites in the four words of this thread's group column (its two
+// rows lie in the same block row) at the black plane z and at the white plane z-1; the other sites
+// keep their old value (they are the frozen halo of the blocks being updated).
+//   DCB = 1 (01 cycle, D14): the blocks of one coarse colour.
+//   DCB = 2 (mixed cycle, D15): the blocks of one coarse colour whose drawn first fine colour is the
+//           launch's `first` (bit array ff from block_order_kernel); the launch's role order (black
+//           role = colour `first`) is then each of these blocks' own order.
+__device__ __forceinline__ uint4 keep_unmasked(const uint4 upd, const uint4 old, const uint4 m)
 {
-    return make_uint4((upd.x & m) | (old.x & ~m), (upd.y & m) | (old.y & ~m), (upd.z & m) | (old.z & ~m),
-                      (upd.w & m) | (old.w & ~m));
+    return make_uint4((upd.x & m.x) | (old.x & ~m.x), (upd.y & m.y) | (old.y & ~m.y),
+                      (upd.z & m.z) | (old.z & ~m.z), (upd.w & m.w) | (old.w & ~m.w));
 }
 
-template <int R4, int PLANE, int U, bool DCB>
+// bit n of the byte -> nibble n of the word (a block of edge 8 spans four bits of a packed word)
+__device__ __forceinline__ uint32_t byte_to_nibbles(uint32_t x)
+{
+    x = (x | (x << 12)) & 0x000F000Fu;
+    x = (x | (x << 6)) & 0x03030303u;
+    x = (x | (x << 3)) & 0x11111111u;
+    return x * 0xFu;
+}
+
+template <int R4, int PLANE, int U, int DCB>
 __device__ __forceinline__ void f2_step(F2Win &w, const F2Ctx &c, const int k, const uint32_t qb,
                                         const uint32_t qw, const uint32_t lap_parity,
-                                        const SweepConsts &keys, const uint32_t mB, const uint32_t mW)
+                                        const SweepConsts &keys, const uint4 mB, const uint4 mW)
 {
     constexpr int S = kF2Stages;
     constexpr int PH = U % 3, O = U & 1;
@@ -236,13 +249,16 @@ __host__ __device__ constexpr int f2_row_lanes(int r4) { return r4 <= 1 ? 1 : r4
 // Grid: blockIdx.x = y tile (RPT stored rows each, RPT even), blockIdx.y = z chunk.
 // Chunk boundaries are odd planes, so the first marched plane z0 = zs-3 is even and the
 // in-row direction of the even tile row at step k is k & 1.
-// DCB: `coarse` = the coarse colour updated by this launch (a double-checkerboard sweep is the launch
-// for coarse 0 followed by the one for coarse 1, each dark sites then light sites, D14).
-template <int R4, int NT, bool DCB>
+// DCB: `coarse` = the coarse colour updated by this launch.  01 cycle (DCB = 1, D14): a sweep is the
+// launch for coarse 0 followed by the one for coarse 1, each dark sites then light sites.  Mixed
+// cycle (DCB = 2, D15): for each coarse colour in the drawn order, one launch with first = 0 and one
+// with first = 1, each masked to the blocks that drew that fine order (ff: bit Bi of the block-order
+// array of this sweep, word (bz nB + by) R4 + x4 for the 32 blocks a group column spans).
+template <int R4, int NT, int DCB>
 __global__ void __launch_bounds__(NT, 2)
 fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, const int L,
                     const int RPT, const int nzc, const int first, const int coarse,
-                    const __grid_constant__ SweepConsts keys)
+                    const uint32_t *__restrict__ ff, const __grid_constant__ SweepConsts keys)
 {
     // R4 = groups per row (L / 256); a row takes RL = the next power of two lanes of a warp (L = 1536:
     // 6 groups on 8 lanes; the two spare lanes of a row repeat its last group and store nothing)
@@ -355,15 +371,25 @@ fused2_sweep_kernel(const uint4 *__restrict__ src, uint4 *__restrict__ dst, cons
     uint32_t qw = (uint32_t)(z == 0 ? L - 1 : z - 1) * c.qplane + c.qrow;
     // double checkerboard: bits j of a word with ((j >> 2) + (y >> 3) + (z >> 3)) & 1 == coarse (philox.cuh)
     const uint32_t ycoarse = DCB ? (uint32_t)((y >> 3) + coarse) : 0u;
-    uint32_t mB = 0xFFFFFFFFu, mW = 0xFFFFFFFFu;
+    const uint32_t ffrow = DCB == 2 ? (uint32_t)(y >> 3) * (uint32_t)R4 + (uint32_t)x4 : 0u;
+    const uint32_t ffplane = (uint32_t)(L >> 3) * (uint32_t)R4;          // ff words per block plane
+    uint4 mB = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu), mW = mB;
 
 #define F2_STEP(U)                                                            \
     {                                                                         \
         if (k >= K) break;                                                    \
         if (DCB) {                                                            \
-            const int zw = z == 0 ? L - 1 : z - 1;                            \
-            mB = ((ycoarse + (uint32_t)(z >> 3)) & 1u) ? 0xF0F0F0F0u : 0x0F0F0F0Fu;  \
-            mW = ((ycoarse + (uint32_t)(zw >> 3)) & 1u) ? 0xF0F0F0F0u : 0x0F0F0F0Fu; \
+            mW = mB;                  /* the white plane z-1 was the previous step's black plane */ \
+            const uint32_t odd = (ycoarse + (uint32_t)(z >> 3)) & 1u;         \
+            if (DCB == 1) {                                                   \
+                const uint32_t m = odd ? 0xF0F0F0F0u : 0x0F0F0F0Fu;           \
+                mB = make_uint4(m, m, m, m);                                  \
+            } else {                                                          \
+                uint32_t fw = __ldg(ff + (uint32_t)(z >> 3) * ffplane + ffrow);  \
+                fw = (first ? fw : ~fw) & (odd ? 0xAAAAAAAAu : 0x55555555u);  \
+                mB = make_uint4(byte_to_nibbles(fw & 0xFFu), byte_to_nibbles((fw >> 8) & 0xFFu),  \
+                                byte_to_nibbles((fw >> 16) & 0xFFu), byte_to_nibbles(fw >> 24));   \
+            }                                                                 \
         }                                                                     \
         f2_step<R4, PLANE, U, DCB>(w, c, k, qb, qw, lap_parity, keys, mB, mW); \
         __syncthreads();                                                      \
@@ -395,17 +421,23 @@ inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
     constexpr int TY = 2 * NT / f2_row_lanes(R4);
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
-    cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, false>,
+    cudaError_t e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, 0>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, true>,
+        e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, 1>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(fused2_sweep_kernel<R4, NT, 2>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int occ = 0, occ_dcb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT, false>, NT, smem);
+    int occ = 0, occ1 = 0, occ2 = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fused2_sweep_kernel<R4, NT, 0>, NT, smem);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_dcb, fused2_sweep_kernel<R4, NT, true>, NT, smem);
-    if (occ_dcb < occ) occ = occ_dcb;          // one launch shape for both
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, fused2_sweep_kernel<R4, NT, 1>, NT, smem);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, fused2_sweep_kernel<R4, NT, 2>, NT, smem);
+    if (occ1 < occ) occ = occ1;                // one launch shape for all three
+    if (occ2 < occ) occ = occ2;
     if (e != cudaSuccess) return e;
     if (occ < 1) occ = 1;
     const int tyo = TY - 4;                        // stored rows per tile (even)
@@ -425,20 +457,25 @@ inline cudaError_t plan_fused2_t(FusedPlan &plan, int L, int sm_count)
 
 template <int R4, int NT>
 inline cudaError_t launch_fused2_t(const uint32_t *src, uint32_t *dst, int L, int first, int coarse,
-                                   const SweepConsts &keys, const FusedPlan &plan, cudaStream_t stream)
+                                   const uint32_t *ff, const SweepConsts &keys, const FusedPlan &plan,
+                                   cudaStream_t stream)
 {
     constexpr int TY = 2 * NT / f2_row_lanes(R4);
     constexpr int PLANE = TY * R4;
     constexpr size_t smem = (size_t)PLANE * 16 * (2 * kF2Stages + 2) + kF2Stages * 8;
     dim3 grid((unsigned)plan.nty, (unsigned)plan.nzc);
     if (coarse < 0)
-        fused2_sweep_kernel<R4, NT, false><<<grid, NT, smem, stream>>>(
+        fused2_sweep_kernel<R4, NT, 0><<<grid, NT, smem, stream>>>(
             reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
-            first, 0, keys);
+            first, 0, nullptr, keys);
+    else if (!ff)
+        fused2_sweep_kernel<R4, NT, 1><<<grid, NT, smem, stream>>>(
+            reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
+            first, coarse, nullptr, keys);
     else
-        fused2_sweep_kernel<R4, NT, true><<<grid, NT, smem, stream>>>(
+        fused2_sweep_kernel<R4, NT, 2><<<grid, NT, smem, stream>>>(
             reinterpret_cast<const uint4 *>(src), reinterpret_cast<uint4 *>(dst), L, plan.RPT, plan.nzc,
-            first, coarse, keys);
+            first, coarse, ff, keys);
     return cudaGetLastError();
 }
 
@@ -455,18 +492,19 @@ inline cudaError_t plan_fused2(FusedPlan &plan, int L, int sm_count)
 }
 
 // coarse < 0: the plain checkerboard sweep; coarse = 0 / 1: the double-checkerboard launch that
-// updates that coarse colour only (D14).
+// updates that coarse colour only (D14), or with ff (the sweep's block-order bits, D15) only its
+// blocks whose first fine colour is `first`.
 inline cudaError_t launch_fused2_sweep(const uint32_t *src, uint32_t *dst, int L, uint32_t t,
                                        uint64_t seed, int first, const FusedPlan &plan,
-                                       cudaStream_t stream, int coarse = -1)
+                                       cudaStream_t stream, int coarse = -1, const uint32_t *ff = nullptr)
 {
     const SweepConsts keys = make_sweep_consts(seed, t, first);
     switch (L) {
-        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, coarse, keys, plan, stream);
-        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, coarse, keys, plan, stream);
-        case 1536: return launch_fused2_t<6, 256>(src, dst, L, first, coarse, keys, plan, stream);
-        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, coarse, keys, plan, stream);
-        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, coarse, keys, plan, stream);
+        case 512:  return launch_fused2_t<2, 128>(src, dst, L, first, coarse, ff, keys, plan, stream);
+        case 1024: return launch_fused2_t<4, 256>(src, dst, L, first, coarse, ff, keys, plan, stream);
+        case 1536: return launch_fused2_t<6, 256>(src, dst, L, first, coarse, ff, keys, plan, stream);
+        case 2048: return launch_fused2_t<8, 256>(src, dst, L, first, coarse, ff, keys, plan, stream);
+        case 4096: return launch_fused2_t<16, 256>(src, dst, L, first, coarse, ff, keys, plan, stream);
         default:   return cudaErrorInvalidValue;
     }
 }

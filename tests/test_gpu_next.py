@@ -228,7 +228,7 @@ def _check_radial(got, want, rep=0):
 
 
 @pytest.mark.parametrize("L,seed,sweeps", [(64, 1, 0), (64, 1, 12), (128, 7, 5), (192, 8, 3), (256, 2, 20),
-                                           (512, 11, 6)])
+                                           (384, 11, 6)])
 def test_radial_estimator_against_oracle(B, orc, L, seed, sweeps):
     sim = B.Ising3D(L, [seed])
     ref = orc.Oracle(L, seed)
@@ -419,38 +419,41 @@ def test_double_checkerboard_batch_neel_and_errors(B, orc):
     sim.free()
 
 
-@pytest.mark.parametrize("L,seed", [(1024, 21), (2048, 22)])
-def test_double_checkerboard_fused2_full_size(B, orc, L, seed):
-    """The masked fused2 launches (one per coarse colour) against the masked generic kernel word for
-    word, from the iid start and from a late-time-like state, and sampled sites against the oracle:
-    a site is recomputed through the four masked half-sweeps of one sweep by brute force."""
+@pytest.mark.parametrize("L,seed,mixed", [(1024, 21, 0), (2048, 22, 0), (1024, 23, 1), (2048, 24, 1)])
+def test_double_checkerboard_fused2_full_size(B, orc, L, seed, mixed):
+    """The masked fused2 launches (01 cycle: one per coarse colour; mixed cycle: one per coarse colour
+    and drawn fine order) against the masked generic kernel word for word, and at L = 1024 against
+    the whole-lattice oracle from the iid start and from a late-time-like state."""
+    cyc = B.CYCLE_DOUBLE_CB_MIXED if mixed else B.CYCLE_DOUBLE_CB
     a = B.Ising3D(L, [seed])
-    a.set_cycle(B.CYCLE_DOUBLE_CB)
+    a.set_cycle(cyc)
     b = B.Ising3D(L, [seed], variant=B.VARIANT_GENERIC)
-    b.set_cycle(B.CYCLE_DOUBLE_CB)
+    b.set_cycle(cyc)
     assert a.variant_name == "fused2" and b.variant_name == "generic"
-    a.sweep(3)
-    b.sweep(3)
+    a.sweep(2)
+    b.sweep(2)
     assert np.array_equal(a.get_state(), b.get_state())
     if L == 1024:
         ref = orc.Oracle(L, seed)
-        ref.sweep_dcb(3, block=8)
+        step = (lambda n: ref.sweep_dcb_mixed(n, block=8)) if mixed else (lambda n: ref.sweep_dcb(n, block=8))
+        step(2)
         assert np.array_equal(a.get_state(), ref.export_words())
         words = inputs.coarse_words(L, 5, block=16)
         a.set_state(words, 700)
         ref.import_words(words, 700)
-        a.sweep(2)
-        ref.sweep_dcb(2, block=8)
+        a.sweep(1)
+        step(1)
         assert np.array_equal(a.get_state(), ref.export_words())
     a.free()
     b.free()
 
 
-@pytest.mark.parametrize("L,seed,cps", [(64, 1, [1, 2, 6]), (128, 7, [1, 4]), (192, 8, [2]), (512, 11, [1, 2])])
-def test_double_checkerboard_mixed_against_oracle(B, orc, L, seed, cps):
-    sim = B.Ising3D(L, [seed])
+@pytest.mark.parametrize("L,seed,variant,cps", [(64, 1, "auto", [1, 2, 6]), (128, 7, "auto", [1, 4]), (192, 8, "auto", [2]),
+                                                (512, 11, "auto", [1, 2, 5]), (512, 12, "generic", [1, 3])])
+def test_double_checkerboard_mixed_against_oracle(B, orc, L, seed, variant, cps):
+    sim = B.Ising3D(L, [seed], variant=VARIANTS(B)[variant])
     sim.set_cycle(B.CYCLE_DOUBLE_CB_MIXED)
-    assert sim.variant_name == "generic"
+    assert sim.variant_name == ("fused2" if (L >= 512 and variant == "auto") else "generic")
     ref = orc.Oracle(L, seed)
     t = 0
     for cp in cps:

