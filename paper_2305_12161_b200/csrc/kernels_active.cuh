@@ -160,14 +160,16 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
     uint32_t *aw_oth = awake + (size_t)(1 - c) * (geo.G >> 5);
     const uint32_t n_chunks = geo.G / kActiveChunk;
     uint32_t evaluated = 0, changed = 0;
+    const uint8_t *flag_bytes = reinterpret_cast<const uint8_t *>(aw_own);
     if (tid == 0) ticket[0] = atomicAdd(tickets, 1u) - base_ticket;
     __syncthreads();
+    // one flag byte (8 groups) per thread; the next chunk's byte is fetched while this chunk is evaluated
+    uint32_t f_next = ticket[0] < n_chunks ? flag_bytes[(size_t)ticket[0] * (kActiveChunk / 8) + tid] : 0u;
     for (int par = 0;; par ^= 1) {
         const uint32_t chunk = ticket[par];
         if (chunk >= n_chunks) break;
-        if (tid == 0) ticket[par ^ 1] = atomicAdd(tickets, 1u) - base_ticket;   // read after the barriers below
-        // one flag byte (8 groups) per thread
-        const uint32_t f = reinterpret_cast<const uint8_t *>(aw_own)[(size_t)chunk * (kActiveChunk / 8) + tid];
+        if (tid == 0) ticket[par ^ 1] = atomicAdd(tickets, 1u) - base_ticket;   // read after the barrier below
+        const uint32_t f = f_next;
         uint32_t incl = __popc(f);
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -177,6 +179,10 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
         if (lane == 31) wtot[warp] = incl;
         if (tid < kActiveChunk / 32) keep[tid] = 0u;
         __syncthreads();
+        {
+            const uint32_t nxt = ticket[par ^ 1];
+            f_next = nxt < n_chunks ? flag_bytes[(size_t)nxt * (kActiveChunk / 8) + tid] : 0u;
+        }
         uint32_t p = incl - __popc(f), total = 0;
 #pragma unroll
         for (int w = 0; w < kActiveThreads / 32; ++w) {
