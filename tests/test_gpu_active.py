@@ -214,7 +214,7 @@ def test_active_equals_fused2_at_full_size_late_time(B, orc):
 @pytest.mark.slow
 def test_auto_run_equals_fused2_run_config4(B):
     """Config 4 (L = 1024, seed 3, 10^5 sweeps) run twice: under the AUTO policy (fused2, probes every
-    1024 sweeps, hand-over to the activity-driven kernel when under 7.5 % of the groups can change)
+    1024 sweeps, hand-over to the activity-driven kernel when under 9 % of the groups can change)
     and on fused2 alone.  Every word of the final states and all counts must agree, and AUTO must
     have handed over on the way."""
     L, seed, n = 1024, 3, 100_000
@@ -223,11 +223,75 @@ def test_auto_run_equals_fused2_run_config4(B):
     a.sweep(n)
     b.sweep(n)
     assert a.variant_name == "active" and b.variant_name == "fused2"
-    assert 0.0 < a.last_activity < 0.075
+    assert 0.0 < a.last_activity < 0.09
     ev = a.active_stats()[0]
     assert ev[0] > 0 and ev[1] > 0
     assert np.array_equal(a.get_state(), b.get_state())
     ma, mb = a.measure(), b.measure()
     assert int(ma["n_up"][0]) == int(mb["n_up"][0]) and np.array_equal(ma["antipar"], mb["antipar"])
+    a.free()
+    b.free()
+
+
+def test_auto_policy_batch_of_two(B, orc):
+    """Two replicas in one handle at L = 512 under AUTO: the hand-over follows the mean awake
+    fraction, each replica keeps its own trajectory (seed) and equals the oracle."""
+    L, seeds = 512, [51, 52]
+    sim = B.Ising3D(L, seeds)
+    sim.set_activity_policy(3, 0.6, 0.95)
+    w = [inputs.pack_spins(inputs.domain_spins(L, 21, block=32, p_minority=0.25, noise=0.0005)),
+         inputs.coarse_words(L, 22, block=16)]
+    sim.set_state(np.concatenate(w), 40)
+    refs = [orc.Oracle(L, s, init=False) for s in seeds]
+    for r, ww in zip(refs, w):
+        r.import_words(ww, 40)
+    sim.sweep(8)
+    assert sim.variant_name == "active"
+    got = sim.get_state().reshape(2, -1)
+    for i, r in enumerate(refs):
+        r.sweep(8)
+        assert np.array_equal(got[i], r.export_words()), "replica %d" % i
+    cnt, frac = sim.activity()
+    for i, r in enumerate(refs):
+        assert list(cnt[i]) == list(r.activity())
+    assert 0.0 < frac < 0.6
+    sim.free()
+
+
+def test_active_equals_fused2_L4096(B):
+    """The largest size (6.9e10 spins, rows of 16 groups, group indices up to 2^28): the activity-driven
+    kernel against fused2 word for word, from a state 30 sweeps into the quench (most groups awake)
+    and from the all-up state with a handful of reversed words (a few groups awake)."""
+    import torch
+    L = 4096
+    nw = L ** 3 // 32
+    a = B.Ising3D(L, [8], variant=B.VARIANT_FUSED2)
+    b = B.Ising3D(L, [8], variant=B.VARIANT_ACTIVE)
+    a.sweep(30)
+    buf = torch.empty(nw, dtype=torch.int32, device="cuda")
+    a.get_state_device(buf.data_ptr(), nw)
+    b.set_state_device(buf.data_ptr(), nw, 30)
+    a.sweep(2)
+    b.sweep(2)
+    a.get_state_device(buf.data_ptr(), nw)
+    ref = buf.clone()
+    b.get_state_device(buf.data_ptr(), nw)
+    b.sync()
+    assert torch.equal(ref, buf)
+    # sparse: all up, then reversed words at the first and last group of each colour and in the middle
+    buf.fill_(-1)
+    idx = torch.tensor([0, 5, nw // 2 - 1, nw // 2, nw // 2 + 7, nw - 1, nw // 3, 3 * (nw // 4) + 2], device="cuda")
+    buf[idx] = 0x0F0F1234
+    a.set_state_device(buf.data_ptr(), nw, 100)
+    b.set_state_device(buf.data_ptr(), nw, 100)
+    cnt, frac = b.activity()
+    assert 0 < int(cnt.sum()) < 200
+    a.sweep(5)
+    b.sweep(5)
+    a.get_state_device(buf.data_ptr(), nw)
+    ref = buf.clone()
+    b.get_state_device(buf.data_ptr(), nw)
+    b.sync()
+    assert torch.equal(ref, buf)
     a.free()
     b.free()
