@@ -246,7 +246,7 @@ int ising3d_active_stats(ising3d_t *h, uint64_t *evaluated_changed);
  * fraction of groups that can change is below `on_below` the following sweeps run on the
  * activity-driven kernel, which hands back to fused2 if the same fraction, probed every
  * probe_interval sweeps, passes `off_above`.  The choice changes the speed only, never the
- * result.  probe_interval = 0: always fused2.  Defaults: 1024, 0.09, 0.12 (measured break-even
+ * result.  probe_interval = 0: always fused2.  Defaults: 1024, 0.11, 0.14 (measured break-even
  * of the two kernels at L = 2048).
  * Each probe / check synchronises the stream once.  EINVAL unless 0 <= on_below <= off_above <= 1.
  */

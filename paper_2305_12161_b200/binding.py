@@ -192,7 +192,7 @@ class Ising3D:
     def set_cluster_size(self, cs: int):
         _check(self._l.ising3d_set_cluster_size(self._h, int(cs)))
 
-    def set_activity_policy(self, probe_interval: int, on_below: float = 0.09, off_above: float = 0.12):
+    def set_activity_policy(self, probe_interval: int, on_below: float = 0.11, off_above: float = 0.14):
         _check(self._l.ising3d_set_activity_policy(self._h, int(probe_interval), float(on_below), float(off_above)))
 
     def activity(self):

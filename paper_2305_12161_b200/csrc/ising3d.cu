@@ -92,7 +92,7 @@ struct ising3d {
     bool active_mode = false;                  // AUTO: the activity-driven kernel is the one being dispatched
     uint64_t run_len = 0;                      // sweeps since the last probe / check (AUTO)
     uint64_t probe_interval = 1024;            // AUTO: dense sweeps between two activity probes (0 = never)
-    double active_on = 0.09, active_off = 0.12;   // AUTO: switch on below / off above this awake fraction
+    double active_on = 0.11, active_off = 0.14;   // AUTO: switch on below / off above this awake fraction
     double last_activity = -1.0;               // awake fraction seen by the last probe / check
 
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }

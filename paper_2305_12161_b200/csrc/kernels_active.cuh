@@ -20,9 +20,11 @@
 // (D5), drawn only for groups that hold a tie, so the trajectory is bit-identical to the dense
 // kernels'.
 //
-// Work distribution: a CTA draws chunks of 2048 consecutive groups (32 KB of each colour) from a
-// ticket counter, compacts the set flag bits into a shared-memory list (one flag byte per thread,
-// CTA-wide prefix sum) and its 256 threads evaluate the listed groups.
+// Work distribution: a CTA draws bricks of 2048 groups (32 rows x 8 planes x all x at L = 2048:
+// compact in y and z, so that the y+-1 and z+-1 words of one evaluation are the same-position
+// words of the evaluations around it and come from L1) from a ticket counter, compacts the set
+// flag bits into a shared-memory list (one flag byte per thread, CTA-wide prefix sum) and its 256
+// threads evaluate the listed groups.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -38,6 +40,9 @@ struct ActiveGeom {
     int lgL;          // L = 1 << lgL
     int lgR4;         // 128-spin groups per row R4 = L / 256 = 1 << lgR4
     uint32_t G;       // groups per colour = L * L * R4
+    // work item of active_halfsweep_kernel: a brick of 2048 groups = PB planes x RB rows x all R4 groups
+    int lgRS;         // groups per plane strip RS = RB * R4, RB = 32 rows
+    int lgPB;         // planes per brick PB = 2048 / RS
 };
 
 inline ActiveGeom make_active_geom(int L)
@@ -47,6 +52,8 @@ inline ActiveGeom make_active_geom(int L)
     while ((1 << g.lgL) < L) ++g.lgL;
     g.lgR4 = g.lgL - 8;
     g.G = (uint32_t)L * (uint32_t)L * (uint32_t)(L >> 8);
+    g.lgRS = g.lgR4 + 5;
+    g.lgPB = 11 - g.lgRS;
     return g;
 }
 
@@ -137,7 +144,7 @@ constexpr int kActiveChunk = 2048;       // groups per work item: 64 flag words 
 
 // ROLE = 0 / 1: first / second colour of the sweep (c = first ^ ROLE; keys.c1[ROLE] carries c).
 // stat[0] += groups evaluated, stat[1] += groups changed.
-// Work items (chunks of 2048 consecutive groups) are handed out through a ticket counter that is
+// Work items (bricks of 2048 groups) are handed out through a ticket counter that is
 // never reset: this launch owns tickets base .. base + n_chunks - 1 (mod 2^32), and every CTA draws
 // exactly one ticket beyond them before it stops, so the next launch starts at
 // base + n_chunks + gridDim.x (the host keeps count).
@@ -161,10 +168,23 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
     const uint32_t n_chunks = geo.G / kActiveChunk;
     uint32_t evaluated = 0, changed = 0;
     const uint8_t *flag_bytes = reinterpret_cast<const uint8_t *>(aw_own);
+    // brick `chunk` = strip by (RB rows) of slab bz (PB planes); its groups are, plane by plane, RS
+    // consecutive group indices from brick_base(chunk) + j * GP
+    const uint32_t RS = 1u << geo.lgRS, GP = 1u << (geo.lgL + geo.lgR4);
+    const int lg_ny = geo.lgL + geo.lgR4 - geo.lgRS;                  // strips per plane = L / RB
+    auto brick_base = [&](uint32_t chunk) -> uint32_t {
+        const uint32_t by = chunk & ((1u << lg_ny) - 1u), bz = chunk >> lg_ny;
+        return ((bz << geo.lgPB) * GP) + (by << geo.lgRS);
+    };
+    // one flag byte (8 groups) per thread: plane fj of the brick, byte fb of its strip
+    const uint32_t fj = (uint32_t)tid >> (geo.lgRS - 3), fb = (uint32_t)tid & ((RS >> 3) - 1u);
+    auto flag_byte = [&](uint32_t chunk) -> uint32_t {
+        return chunk < n_chunks ? flag_bytes[((size_t)brick_base(chunk) + (size_t)fj * GP) / 8 + fb] : 0u;
+    };
     if (tid == 0) ticket[0] = atomicAdd(tickets, 1u) - base_ticket;
     __syncthreads();
-    // one flag byte (8 groups) per thread; the next chunk's byte is fetched while this chunk is evaluated
-    uint32_t f_next = ticket[0] < n_chunks ? flag_bytes[(size_t)ticket[0] * (kActiveChunk / 8) + tid] : 0u;
+    // the next brick's byte is fetched while this brick is evaluated
+    uint32_t f_next = flag_byte(ticket[0]);
     for (int par = 0;; par ^= 1) {
         const uint32_t chunk = ticket[par];
         if (chunk >= n_chunks) break;
@@ -179,10 +199,8 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
         if (lane == 31) wtot[warp] = incl;
         if (tid < kActiveChunk / 32) keep[tid] = 0u;
         __syncthreads();
-        {
-            const uint32_t nxt = ticket[par ^ 1];
-            f_next = nxt < n_chunks ? flag_bytes[(size_t)nxt * (kActiveChunk / 8) + tid] : 0u;
-        }
+        f_next = flag_byte(ticket[par ^ 1]);
+        const uint32_t base = brick_base(chunk);
         uint32_t p = incl - __popc(f), total = 0;
 #pragma unroll
         for (int w = 0; w < kActiveThreads / 32; ++w) {
@@ -196,8 +214,8 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
         for (uint32_t ff = f; ff; ff &= ff - 1) list[p++] = (uint16_t)(tid * 8 + (__ffs(ff) - 1));
         __syncthreads();
         for (uint32_t i = tid; i < total; i += kActiveThreads) {
-            const uint32_t li = list[i];
-            const uint32_t g = chunk * kActiveChunk + li;
+            const uint32_t li = list[i];                     // plane (li >> lgRS) of the brick, group li & (RS - 1) of its strip
+            const uint32_t g = base + (li >> geo.lgRS) * GP + (li & (RS - 1u));
             const GroupNbr n = group_neighbours(g, c, geo);
             const GroupEval e = eval_group(own, oth, g, n);
             uint4 nw = e.det;
@@ -228,7 +246,10 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
             }
         }
         __syncthreads();
-        if (tid < kActiveChunk / 32) aw_own[(size_t)chunk * (kActiveChunk / 32) + tid] = keep[tid];
+        if (tid < kActiveChunk / 32) {
+            const uint32_t bit0 = 32u * (uint32_t)tid;        // first list index of this flag word
+            aw_own[(base + (bit0 >> geo.lgRS) * GP + (bit0 & (RS - 1u))) >> 5] = keep[tid];
+        }
         if (tid == 0) evaluated += total;
     }
     for (int d = 16; d; d >>= 1) changed += __shfl_xor_sync(0xffffffffu, changed, d);

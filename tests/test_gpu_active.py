@@ -214,7 +214,7 @@ def test_active_equals_fused2_at_full_size_late_time(B, orc):
 @pytest.mark.slow
 def test_auto_run_equals_fused2_run_config4(B):
     """Config 4 (L = 1024, seed 3, 10^5 sweeps) run twice: under the AUTO policy (fused2, probes every
-    1024 sweeps, hand-over to the activity-driven kernel when under 9 % of the groups can change)
+    1024 sweeps, hand-over to the activity-driven kernel when under 11 % of the groups can change)
     and on fused2 alone.  Every word of the final states and all counts must agree, and AUTO must
     have handed over on the way."""
     L, seed, n = 1024, 3, 100_000
@@ -223,7 +223,7 @@ def test_auto_run_equals_fused2_run_config4(B):
     a.sweep(n)
     b.sweep(n)
     assert a.variant_name == "active" and b.variant_name == "fused2"
-    assert 0.0 < a.last_activity < 0.09
+    assert 0.0 < a.last_activity < 0.11
     ev = a.active_stats()[0]
     assert ev[0] > 0 and ev[1] > 0
     assert np.array_equal(a.get_state(), b.get_state())
