@@ -295,6 +295,10 @@ def test_radial_estimator_L2048_rounding_margin(B):
     """D12 claims the inverse transform of +-1 data at L = 2048 is within 1e-3 of an integer multiple of
     N, so llrint recovers P(d) exactly: measured here (64 GiB field + cuFFT work area), together with
     the identities that hold at any size."""
+    import gc
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()          # 128 GiB are needed: give back what torch cached for earlier tests
     L = 2048
     sim = B.Ising3D(L, [4])
     sim.sweep(20)
