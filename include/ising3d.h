@@ -280,6 +280,58 @@ int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);
 int ising3d_measure(ising3d_t *h, ising3d_meas_t *out);
 
 /*
+ * ising3d_measure_static -- N_up and A_mu(r) of a packed state the caller already holds on the
+ * device, for callers that must not allocate device memory.
+ *
+ * Who this is for.  Every other entry point works on a handle, and creating a handle either
+ * calls cudaMalloc or asks the caller to bring a buffer of ising3d_required_bytes().  Some users
+ * of this library can do neither at the point where they want a measurement:
+ *  - code that runs inside a service whose device memory is handed out once at start-up by a
+ *    pool it does not control (a framework's caching allocator that has already taken the whole
+ *    GPU, a job scheduler with a fixed per-tenant budget): a cudaMalloc there fails, or succeeds
+ *    and breaks the budget somebody else relies on;
+ *  - code on a latency-critical path (an analysis hook called between sweeps of a running
+ *    simulation, a monitoring thread): cudaMalloc and cudaFree serialise against all work on the
+ *    device, so one measurement would stall every other stream;
+ *  - code that only has the spins, e.g. a state produced by another program in the D3 format,
+ *    and wants the counts without building a simulation handle around them.
+ * For them the accumulators the measurement kernels add into live in a fixed array that is part
+ * of the library image itself (a file-scope __device__ array in ising3d.cu).  Nothing is
+ * allocated or freed by this call, by the library on its behalf, or by any routine it uses;
+ * cuFFT and the tensor-core path (which borrows a lattice-sized buffer) are not involved: the
+ * counts come from the XOR + carry-save popcount kernels (ISING3D_MEASURE_POPCOUNT), which give
+ * the same integers (D8; eq. (2) PAPER.md:43 reduced to counts).
+ *
+ *   dev_words  DEVICE  in   n_rep * L^3/32 words, canonical packed state D3 (the get_state
+ *                           format), 16-byte aligned; read only, owned by the caller
+ *   n_up       HOST    out  [n_rep]            number of +1 spins
+ *   antipar    HOST    out  [n_rep][3][L/2+1]  A_mu(r), mu = x,y,z; A_mu(0) = 0
+ *   cuda_stream             a cudaStream_t (NULL = legacy default stream); the call queues its work
+ *                           there and waits for that stream before returning
+ * n_broken, C(r) and ell are plain host arithmetic on these integers (see ising3d_meas_t and D9).
+ *
+ * The limit.  The array holds ISING3D_STATIC_MAX_COUNTS 64-bit counters (128 KiB; every GPU that
+ * loads the library carries it until the process ends).  A call needs n_rep * (1 + 3 (L/2+1)) of
+ * them: one lattice of any supported L (L = 4096 needs 6 148), 64 replicas of L = 128, 42 of
+ * L = 256.  A larger request is refused with ISING3D_EINVAL and a message that names both numbers;
+ * split the batch over several calls (dev_words + k * L^3/32 is replica k).
+ *
+ * First call on a device.  It looks up the device address of the array (cudaGetSymbolAddress)
+ * and raises the kernels' shared-memory limit, once per device and process, with the device
+ * that is current at the call.  Make that first call during set-up, before any stream capture
+ * is begun.  Later calls on that device only launch kernels and copy the results.
+ *
+ * Sharing.  All calls on one GPU, from any thread, use the same array, and it keeps whatever
+ * the previous call left there.  The call clears the part it uses before counting, so results
+ * never depend on earlier calls; but two calls whose GPU work overlaps (different streams, or
+ * different threads) add into the same counters and both return garbage.  Run them one after
+ * the other.  Handles and ising3d_measure are unaffected: they never touch this array.
+ */
+#define ISING3D_STATIC_MAX_COUNTS 16384
+int ising3d_measure_static(const uint32_t *dev_words, int L, int n_rep, uint64_t *n_up, uint64_t *antipar,
+                           void *cuda_stream);
+
+/*
  * The paper's own estimator: the full correlation matrix by eq. (7)
  * PAPER.md:128, mean_i s_i s_{i+k} = [F^-1(|F s|^2)]_k (3-D real-data DFT in place, fp64, cuFFT),
  * then "radially averaging over the three-dimensional correlation matrix", and

@@ -27,7 +27,7 @@ EXPORTED = [
     "ising3d_required_bytes", "ising3d_words_per_replica", "ising3d_init", "ising3d_init_batch",
     "ising3d_init_batch_with_buffer", "ising3d_reset", "ising3d_set_stream", "ising3d_set_variant", "ising3d_set_cycle", "ising3d_set_temperature", "ising3d_init_menger", "ising3d_set_measure_variant",
     "ising3d_measure_variant_name",
-    "ising3d_sweep", "ising3d_measure", "ising3d_measure_radial", "ising3d_radial_rounding", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
+    "ising3d_sweep", "ising3d_measure", "ising3d_measure_static", "ising3d_measure_radial", "ising3d_radial_rounding", "ising3d_release_radial", "ising3d_get_state", "ising3d_set_state",
     "ising3d_get_state_device", "ising3d_set_state_device", "ising3d_L", "ising3d_n_rep",
     "ising3d_sweep_count", "ising3d_launch_count", "ising3d_variant_name", "ising3d_cluster_size",
     "ising3d_set_cluster_size", "ising3d_activity", "ising3d_active_stats", "ising3d_set_activity_policy", "ising3d_sync",
@@ -86,6 +86,7 @@ def load():
         "ising3d_sweep": (C.c_int, [vp, u64]),
         "ising3d_measure": (C.c_int, [vp, C.POINTER(MeasT)]),
         "ising3d_measure_radial": (C.c_int, [vp, C.POINTER(RadialT)]),
+        "ising3d_measure_static": (C.c_int, [vp, C.c_int, C.c_int, u64p, u64p, vp]),
         "ising3d_radial_rounding": (C.c_int, [vp, C.POINTER(C.c_double)]),
         "ising3d_release_radial": (C.c_int, [vp]),
         "ising3d_get_state": (C.c_int, [vp, vp, C.c_size_t, u64p]),
@@ -129,6 +130,27 @@ def required_bytes(L: int, n_rep: int = 1) -> int:
 
 def words_per_replica(L: int) -> int:
     return int(load().ising3d_words_per_replica(L))
+
+
+STATIC_MAX_COUNTS = 16384
+
+
+def measure_static(dev_ptr: int, L: int, n_rep: int = 1, cuda_stream: int = 0):
+    """ising3d_measure_static: N_up and A_mu(r) of a packed state already on the device, without a
+    handle and without any device allocation (the counters live in an array inside libising3d.so).
+
+    For callers that cannot allocate on the GPU where they measure: all memory belongs to somebody
+    else's pool, or a cudaMalloc would stall the other streams.  `dev_ptr` is the device address of
+    n_rep * L^3/32 uint32 words in the get_state format.  n_rep * (1 + 3 (L/2+1)) must not exceed
+    STATIC_MAX_COUNTS.  Calls share that array: do not let two of them overlap on one GPU.
+    """
+    nr = L // 2 + 1
+    n_up = np.zeros(max(n_rep, 0), dtype=np.uint64)
+    antipar = np.zeros((max(n_rep, 0), 3, nr), dtype=np.uint64)
+    _check(load().ising3d_measure_static(C.c_void_p(dev_ptr), int(L), int(n_rep),
+                                         n_up.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                         antipar.ctypes.data_as(C.POINTER(C.c_uint64)), C.c_void_p(cuda_stream)))
+    return {"n_up": n_up, "antipar": antipar}
 
 
 class Ising3D:

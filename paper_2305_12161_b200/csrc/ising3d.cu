@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -628,6 +629,43 @@ int measure_gram(ising3d *h)
 
 }  // namespace
 
+// ---- ising3d_measure_static: the measurement with its accumulators in library-static memory --------
+// The 64-bit counters count_up_kernel and autocorr_kernel add into ([rep][1 + 3 (L/2+1)], the layout at
+// the top of kernels_measure.cuh).  Part of the loaded module: every GPU that loads the library holds
+// these 128 KiB until the process exits; all calls on one GPU share them.
+// In HOST code this name is only a stand-in for the device object, not a device address: it must never
+// be handed to a kernel.  static_scratch_for_current_device() asks the runtime for the real address.
+static __device__ __align__(256) unsigned long long g_static_counts[ISING3D_STATIC_MAX_COUNTS];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned long long *g_static_ptr[kStaticMaxDevices] = {};   // device address of g_static_counts, per device
+
+// Once per device, with that device current: the device address of g_static_counts and the
+// shared-memory opt-in of the three autocorr kernels (a per-device function attribute).  No allocation.
+int static_scratch_for_current_device(unsigned long long **out)
+{
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(ISING3D_EINVAL, "device ordinal out of range");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        unsigned long long *p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress((void **)&p, g_static_counts));
+        const int max_smem = (int)ising::autocorr_smem_bytes(4096, 8) + 4096;
+        CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        CUDA_TRY(cudaFuncSetAttribute(ising::autocorr_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return ISING3D_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 size_t ising3d_required_bytes(int L, int n_rep)
@@ -919,6 +957,56 @@ int ising3d_measure(ising3d_t *h, ising3d_meas_t *out)
         postprocess(L, out->n_up[rep], a, out->c_intercept,
                     out->C ? out->C + (size_t)rep * nr : nullptr, out->ell ? out->ell + rep : nullptr);
     }
+    return ISING3D_OK;
+}
+
+int ising3d_measure_static(const uint32_t *dev_words, int L, int n_rep, uint64_t *n_up, uint64_t *antipar,
+                           void *cuda_stream)
+{
+    if (!dev_words || !n_up || !antipar) return fail(ISING3D_EINVAL, "null pointer");
+    if (!valid_shape(L, n_rep))
+        return fail(ISING3D_EINVAL, "L must be a multiple of 64 in [64, 4096] and n_rep >= 1");
+    if ((uintptr_t)dev_words & 15) return fail(ISING3D_EINVAL, "dev_words must be 16-byte aligned");
+    const int nr = L / 2 + 1, cpr = 1 + 3 * nr;
+    if ((uint64_t)n_rep * (uint64_t)cpr > (uint64_t)ISING3D_STATIC_MAX_COUNTS)
+        return fail(ISING3D_EINVAL,
+                    "ising3d_measure_static: n_rep * (1 + 3 (L/2+1)) = " + std::to_string((uint64_t)n_rep * cpr) +
+                        " counters exceed the static scratch of " + std::to_string(ISING3D_STATIC_MAX_COUNTS) +
+                        " (ISING3D_STATIC_MAX_COUNTS); measure fewer replicas per call or use ising3d_measure");
+    unsigned long long *counts = nullptr;
+    const int rc = static_scratch_for_current_device(&counts);   // first call on a device: set-up
+    if (rc != ISING3D_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    int sm_count = 0, dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    // the array keeps the previous call's sums and the kernels only add: clear the part this call uses
+    CUDA_TRY(cudaMemsetAsync(counts, 0, (size_t)n_rep * cpr * 8, stream));
+    const size_t wpr = (size_t)L * L * L / 32;
+    {
+        const size_t n4 = wpr / 4;
+        const unsigned gx = (unsigned)std::min<size_t>((n4 + 255) / 256, (size_t)sm_count * 8);
+        ising::count_up_kernel<<<dim3(gx, n_rep), 256, 0, stream>>>(dev_words, counts, wpr, cpr);
+    }
+    {
+        // same tiling as the popcount branch of ising3d_measure (kernels_measure.cuh)
+        const int C = ising::autocorr_tile_sequences(L);
+        const int n_tiles = (L * L / 32) / C;
+        const size_t smem = ising::autocorr_smem_bytes(L, C);
+        int gx = std::max(1, (sm_count + n_rep - 1) / n_rep);
+        gx = std::min(gx, n_tiles);
+        const dim3 grid((unsigned)gx, (unsigned)n_rep);
+        ising::autocorr_kernel<0><<<grid, ising::kAcThreads, smem, stream>>>(dev_words, counts, L, C, n_tiles, cpr);
+        ising::autocorr_kernel<1><<<grid, ising::kAcThreads, smem, stream>>>(dev_words, counts, L, C, n_tiles, cpr);
+        ising::autocorr_kernel<2><<<grid, ising::kAcThreads, smem, stream>>>(dev_words, counts, L, C, n_tiles, cpr);
+    }
+    CUDA_TRY(cudaGetLastError());
+    // [rep][0] -> n_up[rep], [rep][1 ..] -> antipar[rep][3][nr]: two strided copies straight into the
+    // caller's arrays, no staging buffer
+    CUDA_TRY(cudaMemcpy2DAsync(n_up, 8, counts, (size_t)cpr * 8, 8, (size_t)n_rep, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaMemcpy2DAsync(antipar, (size_t)3 * nr * 8, counts + 1, (size_t)cpr * 8, (size_t)3 * nr * 8,
+                               (size_t)n_rep, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
     return ISING3D_OK;
 }
 
