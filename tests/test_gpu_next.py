@@ -313,7 +313,12 @@ def test_radial_estimator_L2048_rounding_margin(B):
 
 # ------------------------------------------------------------------ f-4: finite-temperature Glauber
 @pytest.mark.parametrize("L,seed,T,cps", [(64, 1, 4.0, [1, 2, 5]), (64, 2, 1.5, [1, 4]), (64, 3, 0.3, [2]),
-                                          (128, 7, 4.51, [1, 3]), (192, 8, 2.0, [2]), (64, 9, 1e9, [1, 3])])
+                                          (128, 7, 4.51, [1, 3]), (192, 8, 2.0, [2]), (64, 9, 1e9, [1, 3]),
+                                          # L % 256 == 0: the kernel's 128-bit branch (kernels_generic.cuh, WPR % 4 == 0);
+                                          # L = 256 has one 128-spin group per row (previous = next = itself), L = 512 two;
+                                          # T = 0.3 makes p(n = 6) round to 1, i.e. the threshold 2^32 (bit 32 of D13's table)
+                                          (256, 11, 0.3, [1, 3]), (256, 12, 4.51, [1, 2]),
+                                          (512, 13, 0.5, [1, 2]), (512, 14, 3.0, [1, 2])])
 def test_glauber_against_oracle(B, orc, L, seed, T, cps):
     sim = B.Ising3D(L, [seed])
     sim.set_temperature(T)
@@ -333,6 +338,36 @@ def test_glauber_against_oracle(B, orc, L, seed, T, cps):
     ref.sweep(2)
     assert np.array_equal(sim.get_state(), ref.export_words())
     sim.free()
+
+
+@pytest.mark.parametrize("L,T", [(256, 0.5), (256, 4.0), (512, 1.5)])
+def test_glauber_vector_branch_from_coarse_state_and_batch(B, orc, L, T):
+    """The 128-bit branch of the Glauber kernel (L % 256 == 0) on a domain-like state entered through
+    set_state at a late sweep index, every word against orc_sweep_T (eq. (5)); at L = 256
+    also as a batch, whose replicas must equal single lattices."""
+    words = inputs.coarse_words(L, 21, block=16)
+    sim = B.Ising3D(L, [77])
+    sim.set_temperature(T)
+    sim.set_state(words, 12_345)
+    assert sim.variant_name == "glauber"
+    ref = orc.Oracle(L, 77, init=False)
+    ref.import_words(words, 12_345)
+    sim.sweep(2)
+    ref.sweep_T(2, T)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    check_measure(sim.measure(), ref.measure_full())
+    sim.free()
+    if L == 256:
+        seeds = [5, 6]
+        batch = B.Ising3D(L, seeds)
+        batch.set_temperature(T)
+        batch.sweep(2)
+        st = batch.get_state().reshape(2, -1)
+        for i, sd in enumerate(seeds):
+            r = orc.Oracle(L, sd)
+            r.sweep_T(2, T)
+            assert np.array_equal(st[i], r.export_words())
+        batch.free()
 
 
 def test_glauber_batch_and_errors(B, orc):
