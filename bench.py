@@ -48,6 +48,9 @@ def parse():
     ap.add_argument("--no-measure", action="store_true", help="step = reset + sweeps only")
     ap.add_argument("--no-late-windows", action="store_true",
                     help="skip the sweeps-only windows at t = 10^4 and 10^5 of the full run (about 40 s)")
+    ap.add_argument("--profile-sweeps", type=int, default=0,
+                    help="after each sweeps-only window run this many extra sweeps between cudaProfilerStart/Stop "
+                         "(for `ncu --profile-from-start off`; outside every timed region)")
     ap.add_argument("--cpu-sizes", default="256x20,1024x2,2048x1",
                     help="extra oracle timings LxSWEEPS (SURVEY.md 8(d)); empty to skip")
     return ap.parse_args()
@@ -221,15 +224,17 @@ def measured_peak():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)", {}
 
 
-def ncu_traffic(kernel: str, L: int):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed ncu --set full capture (profiles/roofline_traffic.csv); None if not captured."""
+def ncu_row(kernel: str, L: int, t0: int = 0):
+    """The row of profiles/roofline_traffic.csv for (kernel, L, t0): numbers of one launch of that kernel
+    from a committed `ncu --set full` capture -- dram__bytes_read.sum + dram__bytes_write.sum, and
+    smsp__inst_executed.sum over the launch's warp-steps (stated in the capture's .md).  t0 = the sweep index the capture was taken near (the activity-driven
+    kernel's traffic depends on how far the quench is).  None if not captured."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     try:
         for line in open(p).read().splitlines()[1:]:
-            k, l, b, _ = line.split(",")
-            if k == kernel and int(l) == L:
-                return float(b)
+            k, l, t, b, inst, cap = line.split(",")
+            if k == kernel and int(l) == L and int(t) == t0:
+                return {"dram_bytes": float(b), "instr_per_step": float(inst) if inst else None, "capture": cap}
     except Exception:
         pass
     return None
@@ -334,6 +339,16 @@ def run_ours(args):
                "ms_per_step": ems / k_e2e,
                "note": "set_state(pinned host, 1 GiB at L=2048) + sweep + measure(host counts) per step"}
 
+    def profile_sweeps(h, k):
+        torch.cuda.synchronize()
+        torch.cuda.profiler.start()
+        h.sweep(k)
+        torch.cuda.synchronize()
+        torch.cuda.profiler.stop()
+
+    if args.profile_sweeps and world == 1:
+        profile_sweeps(sim, args.profile_sweeps)          # the state after the last step: t = S, still all awake
+
     # ---------------- sweeps-only windows of the full run ----------------
     # t = 0 is the headline window above; the lattice is then taken on to t = 10^4 and 10^5 (AUTO policy:
     # fused2, handing over to the activity-driven kernel once few groups can still change) and `wS` sweeps
@@ -358,6 +373,19 @@ def run_ours(args):
             ms = w0.elapsed_time(w1) / wS
             windows.append({"t0": t0, "sweeps": wS, "ms_per_sweep": ms, "kernel": sim.variant_name,
                             "site_updates_per_ns": N / (ms * 1e6), "awake_group_fraction": frac})
+            if args.profile_sweeps:
+                profile_sweeps(sim, args.profile_sweeps)
+        # per window: the bytes its kernel moved per sweep in the committed ncu capture taken at that t0
+        # (profiles/roofline_traffic.csv), and the fraction of the copy bandwidth that is at this window's speed
+        peak_w = measured_peak()[0]
+        for w in windows:
+            kname, per_sweep = {"fused2": ("fused2_sweep_kernel", 1), "active": ("active_halfsweep_kernel", 2)}.get(
+                w["kernel"], (None, 0))
+            row = ncu_row(kname, L, w["t0"]) if kname else None
+            w["traffic_bytes_per_sweep"] = row["dram_bytes"] * per_sweep if row else None
+            w["frac_on_bytes_moved"] = (row["dram_bytes"] * per_sweep / (w["ms_per_sweep"] * 1e-3) / 1e9 / peak_w
+                                        if row else None)
+            w["traffic_capture"] = row["capture"] if row else None
 
     if rank != 0:
         if world > 1:
@@ -382,10 +410,13 @@ def run_ours(args):
     alu_bound = 148 * 64 * sm_mhz * 1e6 / alu_ops_per_site / 1e9
     hbm_bound = peak / ALGO_BYTES_PER_SITE_UPDATE
     sweep_rate = N * S / (sweep_ms * 1e6)
-    traffic = ncu_traffic(kernel, L)
-    # as compiled (profiles/r1i, ncu smsp__inst_executed.sum): 337 warp-instructions per thread-step of
-    # 4 groups = 512 sites, 60 of 64 tile rows and 256 of 260 planes stored
-    compiled_per_site = 337.0 / 512.0 * (64.0 / 60.0) * (260.0 / 256.0)
+    row = ncu_row(kernel, L)
+    traffic = row["dram_bytes"] if row else None
+    # as compiled: warp-instructions per thread-step of 4 groups = 512 sites = smsp__inst_executed.sum of the
+    # committed capture over the launch's warp-steps (profiles/roofline_traffic.csv, derived in the capture's
+    # .md; 337.9 in r2); 60 of 64 tile rows and 256 of 260 planes stored
+    compiled_instr = row["instr_per_step"] if (row and row["instr_per_step"]) else 337.9
+    compiled_per_site = compiled_instr / 512.0 * (64.0 / 60.0) * (260.0 / 256.0)
     compiled_bound = 148 * 64 * sm_mhz * 1e6 / compiled_per_site / 1e9
     roofline = {
         "bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -397,7 +428,7 @@ def run_ours(args):
         "issue_frac_as_compiled": sweep_rate / compiled_bound if kernel == "fused2_sweep_kernel" else None,
         "issue_model": {"thread_instr_per_clk_per_sm": 64, "sms": 148, "sm_mhz": sm_mhz,
                         "min_instr_per_128_sites_per_colour": 69,
-                        "compiled_warp_instr_per_thread_step_of_512_sites": 337,
+                        "compiled_warp_instr_per_thread_step_of_512_sites": compiled_instr,
                         "source": "microbench/pipe_rates.cu, microbench/sweep_ceiling.cu; profiles/r1c, r1h, r1i"},
         # on the bytes the kernel really moves (ncu dram__bytes_read + write per launch)
         "frac_on_bytes_moved": (traffic / (avg_launch_ms * 1e-3) / 1e9) / peak if traffic else None,

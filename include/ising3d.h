@@ -242,13 +242,19 @@ int ising3d_active_stats(ising3d_t *h, uint64_t *evaluated_changed);
 
 /*
  * Policy of ISING3D_VARIANT_AUTO at L >= 512 (T = 0, plain checkerboard): after every
- * `probe_interval` sweeps the activity flags are rebuilt and counted; if the
- * fraction of groups that can change is below `on_below` the following sweeps run on the
- * activity-driven kernel, which hands back to fused2 if the same fraction, probed every
- * probe_interval sweeps, passes `off_above`.  The choice changes the speed only, never the
- * result.  probe_interval = 0: always fused2.  Defaults: 1024, 0.11, 0.14 (measured break-even
- * of the two kernels at L = 2048).
- * Each probe / check synchronises the stream once.  EINVAL unless 0 <= on_below <= off_above <= 1.
+ * `probe_interval` dense sweeps the activity flags are rebuilt and counted on the stream; once the
+ * fraction of groups that can change has been seen below `on_below`, the following sweeps run on
+ * the activity-driven kernel.  That kernel tallies the groups it finds holding a Delta E <= 0 site;
+ * every probe_interval sweeps the tally is read, and if its mean per colour update passes
+ * `off_above` (as a fraction of the groups of a colour) the handle goes back to fused2.
+ * No probe blocks the host: the counts go to pinned memory, an event marks them, and the library
+ * looks at the event (cudaEventQuery) between launches and at the start of the next ising3d_sweep
+ * call, so a switch takes effect some sweeps after the probe that caused it -- at most one probe is
+ * in flight, and one that the GPU has not reached yet makes the next one be skipped.  The choice
+ * changes the speed only, never the result.  probe_interval = 0: always fused2.  Defaults: 1024,
+ * 0.11, 0.14 (measured break-even of the two kernels at L = 2048).  Changing the
+ * temperature, the cycle, the variant, the policy or the state puts the handle back on fused2.
+ * EINVAL unless 0 <= on_below <= off_above <= 1.
  */
 int ising3d_set_activity_policy(ising3d_t *h, uint64_t probe_interval, double on_below, double off_above);
 
@@ -264,8 +270,10 @@ int ising3d_set_cluster_size(ising3d_t *h, int cs);
 
 /*
  * Run n_sweeps checkerboard sweeps (eq. (6)).
- * Asynchronous on the handle's stream; no host synchronisation inside, except the one per
- * probe_interval sweeps of the AUTO policy at L >= 512 (ising3d_set_activity_policy).
+ * Asynchronous on the handle's stream; no host synchronisation inside, under every variant
+ * and policy (the AUTO policy's probes are queued on the stream and read back through pinned
+ * memory and an event, ising3d_set_activity_policy).  Inside a stream capture the call records
+ * sweeps only, on the kernel the handle was dispatching when the capture began.
  * The sweep counter advances by n_sweeps; EINVAL if it would pass 2^32-1.
  */
 int ising3d_sweep(ising3d_t *h, uint64_t n_sweeps);
@@ -397,7 +405,9 @@ const char *ising3d_measure_variant_name(const ising3d_t *h);
  * kernel is dispatched. */
 int ising3d_cluster_size(const ising3d_t *h);
 
-/* Block until all work queued on the handle's stream is done. */
+/* Block until all work queued on the handle's stream is done.  A probe of the AUTO policy that
+ * was in flight has landed by then and its result is applied (so has it after ising3d_get_state):
+ * ising3d_variant_name and ising3d_activity's last_fraction are up to date afterwards. */
 int ising3d_sync(ising3d_t *h);
 
 /* Release the handle and all memory the library allocated for it. NULL is a no-op. */

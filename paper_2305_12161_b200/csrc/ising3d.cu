@@ -50,6 +50,8 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+constexpr int kActStride = 8;    // 64-bit counters per replica in d_act
+
 struct ising3d {
     int L = 0, n_rep = 0;
     uint64_t sweep = 0;
@@ -85,7 +87,8 @@ struct ising3d {
     bool attr_gram = false, attr_autocorr = false;
     // activity-driven sweeps (kernels_active.cuh): one flag per 128-spin group and colour
     uint32_t *d_awake = nullptr;               // [n_rep][2][G/32]; valid only while flags_valid
-    unsigned long long *d_act = nullptr;       // [n_rep][4]: flag counts of colour 0, 1; groups evaluated, changed
+    unsigned long long *d_act = nullptr;       // [n_rep][kActStride]: flag counts of colour 0, 1; groups evaluated,
+                                               // changed; groups found holding a Delta E <= 0 site (probe tally)
     unsigned int *d_tickets = nullptr;         // work-item counter of active_halfsweep_kernel (never reset)
     uint32_t *d_ff = nullptr;                  // [n_rep][(L/8)^3/32] block-order bits of the current sweep (D15, fused2)
     ising::ActivePlan plan_act;
@@ -95,6 +98,15 @@ struct ising3d {
     uint64_t probe_interval = 1024;            // AUTO: dense sweeps between two activity probes (0 = never)
     double active_on = 0.11, active_off = 0.14;   // AUTO: switch on below / off above this awake fraction
     double last_activity = -1.0;               // awake fraction seen by the last probe / check
+    // AUTO probes never block the host: counts are copied to pinned memory, an event marks the copy,
+    // and the enqueue loop looks at the event (cudaEventQuery) between launches
+    unsigned long long *h_probe = nullptr;     // pinned, [n_rep][kActStride]
+    cudaEvent_t probe_event = nullptr;
+    bool probe_pending = false;                // a probe is in flight on the stream
+    bool probe_stale = false;                  // ... but the state was replaced since: drop its result
+    bool probe_active = false;                 // it was taken in active mode (tally) / dense mode (flag counts)
+    uint64_t probe_sweeps = 0;                 // sweeps the active-mode tally of that probe covers
+    uint64_t tally_sweeps = 0;                 // active-mode sweeps enqueued since the tally was last cleared
 
     size_t words_per_replica() const { return (size_t)L * L * L / 32; }
     size_t state_bytes() const { return words_per_replica() * 4 * (size_t)n_rep; }
@@ -144,6 +156,7 @@ struct ising3d {
         active_mode = false;
         run_len = 0;
         last_activity = -1.0;
+        probe_stale = probe_pending;
     }
     size_t flag_words() const { return (size_t)L * L * (L >> 8) / 32; }   // per colour
     bool use_fused() const
@@ -170,7 +183,7 @@ Layout make_layout(int L, int n_rep)
     l.queue = align_up((size_t)n_rep * 3 * 4, 256);
     const bool act = ising::active_supported(L);
     l.awake = act ? align_up((size_t)n_rep * 2 * ((size_t)L * L * (L >> 8) / 8), 256) : 0;
-    l.act = act ? align_up((size_t)n_rep * 4 * 8, 256) + 256 : 0;        // + the ticket counter
+    l.act = act ? align_up((size_t)n_rep * kActStride * 8, 256) + 256 : 0;        // + the ticket counter
     l.ff = ising::fused2_supported(L) ? align_up((size_t)n_rep * ((size_t)(L / 8) * (L / 8) * (L / 8) / 8), 256) : 0;
     l.total = 2 * l.state + l.seeds + l.counts + l.gsum + l.queue + l.awake + l.act + l.ff;
     return l;
@@ -251,11 +264,20 @@ int create(ising3d_t **out, int L, int n_rep, const uint64_t *seeds, void *dev_b
             code = fail(ISING3D_ECUDA, std::string("setup: ") + cudaGetErrorString(e));
             break;
         }
+        if (h->d_act && lay.ff &&
+            ((e = cudaHostAlloc((void **)&h->h_probe, (size_t)n_rep * kActStride * 8, cudaHostAllocDefault)) != cudaSuccess ||
+             (e = cudaEventCreateWithFlags(&h->probe_event, cudaEventDisableTiming)) != cudaSuccess)) {
+            code = fail(ISING3D_ECUDA, std::string("setup (probe buffer): ") + cudaGetErrorString(e));
+            break;
+        }
         // the seeds vector outlives the copy (it lives in the handle)
         code = launch_init(h);
     } while (0);
     if (code != ISING3D_OK) {
         if (h->owns_mem && h->base) cudaFree(h->base);
+        if (h->h_probe) cudaFreeHost(h->h_probe);
+        if (h->probe_event) cudaEventDestroy(h->probe_event);
+        cudaGetLastError();
         delete h;
         return code;
     }
@@ -423,10 +445,10 @@ int sweep_fused(ising3d *h, uint64_t i0, uint64_t n, bool gen2)
 int build_flags(ising3d *h)
 {
     const size_t wpr = h->words_per_replica(), fw = h->flag_words();
-    CUDA_TRY(cudaMemset2DAsync(h->d_act, 4 * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][0..1]
+    CUDA_TRY(cudaMemset2DAsync(h->d_act, kActStride * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][0..1]
     for (int rep = 0; rep < h->n_rep; ++rep) {
         cudaError_t e = ising::launch_activity_flags(h->state[h->cur] + rep * wpr, h->d_awake + rep * 2 * fw,
-                                                     h->d_act + rep * 4, h->L, h->stream);
+                                                     h->d_act + rep * kActStride, h->L, h->stream);
         if (e != cudaSuccess)
             return fail(ISING3D_ECUDA, std::string("activity flags launch: ") + cudaGetErrorString(e));
     }
@@ -435,20 +457,21 @@ int build_flags(ising3d *h)
     return ISING3D_OK;
 }
 
-// Synchronises the stream.  frac = mean over replicas and colours of d_act[rep][0..1] / G;
+// Synchronises the stream (ising3d_activity only; the AUTO probes go through probe_enqueue / probe_poll).
+// frac = mean over replicas and colours of d_act[rep][0..1] / G;
 // raw[rep][0..1] = the two counts.
 int read_activity(ising3d *h, double *frac, uint64_t *raw)
 {
-    std::vector<unsigned long long> host((size_t)h->n_rep * 4);
+    std::vector<unsigned long long> host((size_t)h->n_rep * kActStride);
     CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_act, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     const double G = (double)h->flag_words() * 32.0;
     double sum = 0.0;
     for (int rep = 0; rep < h->n_rep; ++rep) {
-        sum += (double)host[rep * 4 + 0] + (double)host[rep * 4 + 1];
+        sum += (double)host[rep * kActStride + 0] + (double)host[rep * kActStride + 1];
         if (raw) {
-            raw[rep * 2 + 0] = host[rep * 4 + 0];
-            raw[rep * 2 + 1] = host[rep * 4 + 1];
+            raw[rep * 2 + 0] = host[rep * kActStride + 0];
+            raw[rep * 2 + 1] = host[rep * kActStride + 1];
         }
     }
     if (frac) *frac = sum / (2.0 * G * h->n_rep);
@@ -474,40 +497,118 @@ int sweep_active(ising3d *h, uint64_t i0, uint64_t n)
             const uint64_t seed = h->seeds[rep];
             const int first = h->cycle == ISING3D_CYCLE_MIXED ? ising::first_colour(seed, t) : 0;
             cudaError_t e = ising::launch_active_sweep(h->state[h->cur] + rep * wpr, h->d_awake + rep * 2 * fw,
-                                                       h->d_act + rep * 4 + 2, h->d_tickets, h->plan_act,
+                                                       h->d_act + rep * kActStride + 2, h->d_tickets, h->plan_act,
                                                        h->L, t, seed, first, h->stream);
-            if (e != cudaSuccess)
+            if (e != cudaSuccess) {
+                // a refused launch leaves the host's ticket count and the flags in doubt: start both over
+                ising::reset_active_tickets(h->d_tickets, h->plan_act, h->stream);
+                h->flags_valid = false;
                 return fail(ISING3D_ECUDA, std::string("active sweep launch: ") + cudaGetErrorString(e));
+            }
         }
         h->launches += 2 * (uint64_t)h->n_rep;
     }
     return ISING3D_OK;
 }
 
-// ISING3D_VARIANT_AUTO at L >= 512, T = 0, plain checkerboard: dense fused2 sweeps while most groups
-// still hold a site that can change, the activity-driven kernel once few do.  Every probe_interval
-// sweeps the flags are rebuilt and counted (one stream synchronisation); below active_on the next
-// sweeps run activity-driven, and go back to fused2 if the fraction passes active_off.
+// ---- ISING3D_VARIANT_AUTO at L >= 512, T = 0, plain checkerboard -------------------------------------
+// Dense fused2 sweeps while most groups still hold a site that can change, the activity-driven kernel
+// once few do.  The choice changes the speed only, never the result, so it may lag: nothing here
+// waits for the GPU.  Every probe_interval sweeps a probe is queued on the stream
+//   dense mode:  rebuild the flags and count them (activity_flags_kernel), copy the counts to pinned memory
+//   active mode: copy the kernel's own tally of groups found holding a Delta E <= 0 site, then clear it
+// followed by an event; probe_poll looks at the event between launches and switches mode once a
+// result has landed (on below active_on, off above active_off).  At most one probe is in flight.
+
+// Clear the active-mode tally [rep][4] (stream ordered).
+int clear_tally(ising3d *h)
+{
+    CUDA_TRY(cudaMemset2DAsync(h->d_act + 4, kActStride * 8, 0, 8, (size_t)h->n_rep, h->stream));
+    h->tally_sweeps = 0;
+    return ISING3D_OK;
+}
+
+int probe_poll(ising3d *h)
+{
+    if (!h->probe_pending) return ISING3D_OK;
+    const cudaError_t q = cudaEventQuery(h->probe_event);
+    if (q == cudaErrorNotReady) {
+        cudaGetLastError();
+        return ISING3D_OK;
+    }
+    h->probe_pending = false;
+    if (q != cudaSuccess) return fail(ISING3D_ECUDA, std::string("activity probe: ") + cudaGetErrorString(q));
+    if (h->probe_stale) {                       // taken on a state that has been replaced since
+        h->probe_stale = false;
+        return ISING3D_OK;
+    }
+    const double G = (double)h->flag_words() * 32.0;
+    double sum = 0.0;
+    for (int rep = 0; rep < h->n_rep; ++rep) {
+        const unsigned long long *c = h->h_probe + (size_t)rep * kActStride;
+        sum += h->probe_active ? (double)c[4] : (double)c[0] + (double)c[1];
+    }
+    // dense: flags set / all flags; active: groups that held such a site per colour update / groups per colour
+    const double frac = sum / (2.0 * G * h->n_rep * (h->probe_active ? (double)h->probe_sweeps : 1.0));
+    h->last_activity = frac;
+    if (h->probe_active && h->active_mode && frac > h->active_off) {
+        h->active_mode = false;
+        h->run_len = 0;
+    } else if (!h->probe_active && !h->active_mode && frac < h->active_on) {
+        h->active_mode = true;
+        h->run_len = 0;
+        return clear_tally(h);                 // the tally counts from the first active sweep
+    }
+    return ISING3D_OK;
+}
+
+// Queue one probe after the sweeps enqueued so far.
+int probe_enqueue(ising3d *h)
+{
+    if (h->probe_pending) return ISING3D_OK;   // the GPU has not reached the previous one yet
+    if (h->active_mode && h->tally_sweeps == 0) return ISING3D_OK;
+    const uint64_t sweeps = h->tally_sweeps;
+    if (!h->active_mode) {
+        const int rc = build_flags(h);
+        if (rc != ISING3D_OK) return rc;
+    }
+    CUDA_TRY(cudaMemcpyAsync(h->h_probe, h->d_act, (size_t)h->n_rep * kActStride * 8, cudaMemcpyDeviceToHost,
+                             h->stream));
+    if (h->active_mode) {
+        const int rc = clear_tally(h);
+        if (rc != ISING3D_OK) return rc;
+    }
+    CUDA_TRY(cudaEventRecord(h->probe_event, h->stream));
+    h->probe_pending = true;
+    h->probe_stale = false;
+    h->probe_active = h->active_mode;
+    h->probe_sweeps = sweeps;
+    return ISING3D_OK;
+}
+
 int sweep_auto(ising3d *h, uint64_t n)
 {
+    const uint64_t kPollEvery = 64;            // sweeps enqueued between two looks at the event
+    // inside a stream capture: sweeps only, in the mode the handle is in (no event query, no probe)
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    CUDA_TRY(cudaStreamIsCapturing(h->stream, &cap));
+    const bool probing = cap == cudaStreamCaptureStatusNone;
     uint64_t i = 0;
     while (i < n) {
-        const uint64_t m = std::min<uint64_t>(n - i, h->probe_interval - h->run_len);
-        int rc = h->active_mode ? sweep_active(h, i, m) : sweep_fused(h, i, m, true);
+        int rc = probing ? probe_poll(h) : ISING3D_OK;
+        if (rc != ISING3D_OK) return rc;
+        const uint64_t left = h->run_len < h->probe_interval ? h->probe_interval - h->run_len : 1;
+        const uint64_t m = std::min<uint64_t>(std::min<uint64_t>(n - i, left), kPollEvery);
+        rc = h->active_mode ? sweep_active(h, i, m) : sweep_fused(h, i, m, true);
         if (rc != ISING3D_OK) return rc;
         i += m;
         h->run_len += m;
-        if (h->run_len < h->probe_interval) break;
-        // the same probe in both modes: rebuild the flags (exact: the ones an active run carries also
-        // hold woken groups not evaluated yet) and count the groups that hold a Delta E <= 0 site
-        double frac = 0.0;
-        rc = build_flags(h);
-        if (rc == ISING3D_OK) rc = read_activity(h, &frac, nullptr);
-        if (rc != ISING3D_OK) return rc;
-        if (h->active_mode && frac > h->active_off) h->active_mode = false;
-        else if (!h->active_mode && frac < h->active_on) h->active_mode = true;
-        h->last_activity = frac;
-        h->run_len = 0;
+        if (h->active_mode) h->tally_sweeps += m;
+        if (h->run_len >= h->probe_interval) {
+            rc = probing ? probe_enqueue(h) : ISING3D_OK;
+            if (rc != ISING3D_OK) return rc;
+            h->run_len = 0;
+        }
     }
     return ISING3D_OK;
 }
@@ -728,6 +829,10 @@ int ising3d_set_temperature(ising3d_t *h, double T)
     if (!(T >= 0.0) || !std::isfinite(T)) return fail(ISING3D_EINVAL, "temperature must be finite and >= 0");
     if (T > 0.0 && h->cycle != ISING3D_CYCLE_01)
         return fail(ISING3D_EINVAL, "finite temperature is implemented for the 01 cycle only");
+    if (T != h->temperature) {      // other dynamics from here on: the adaptive choice starts over on the dense kernel
+        h->active_mode = false;
+        h->run_len = 0;
+    }
     h->temperature = T;
     if (T > 0.0) {
         // D13: thr[n] = floor(2^32 / (1 + exp((12 - 4n)/T))), fp64, n = antiparallel neighbours
@@ -757,7 +862,11 @@ int ising3d_set_cycle(ising3d_t *h, int cycle)
     if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_FUSED3)
         return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
     if (cycle >= ISING3D_CYCLE_DOUBLE_CB && h->variant == ISING3D_VARIANT_ACTIVE)
-        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
+    if (cycle != h->cycle) {
+        h->active_mode = false;
+        h->run_len = 0;
+    }
     h->cycle = cycle;
     return ISING3D_OK;
 }
@@ -787,7 +896,7 @@ int ising3d_set_variant(ising3d_t *h, int variant)
     if (variant == ISING3D_VARIANT_ACTIVE && !h->active_ok())
         return fail(ISING3D_EINVAL, "the activity-driven kernel needs L in {256,512,1024,2048,4096}");
     if (variant == ISING3D_VARIANT_ACTIVE && h->cycle >= ISING3D_CYCLE_DOUBLE_CB)
-        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident and generic kernels");
+        return fail(ISING3D_EINVAL, "the double checkerboard runs on the resident, fused2 and generic kernels");
     if (h->cycle == ISING3D_CYCLE_DOUBLE_CB_MIXED && variant != ISING3D_VARIANT_AUTO &&
         variant != ISING3D_VARIANT_GENERIC && variant != ISING3D_VARIANT_FUSED2)
         return fail(ISING3D_EINVAL, "the mixed-cycle double checkerboard runs on the fused2 and generic kernels");
@@ -843,13 +952,13 @@ int ising3d_active_stats(ising3d_t *h, uint64_t *evaluated_changed)
 {
     if (!h || !evaluated_changed) return fail(ISING3D_EINVAL, "null pointer");
     if (!h->active_ok()) return fail(ISING3D_EINVAL, "the activity-driven kernel needs L in {256,512,1024,2048,4096}");
-    std::vector<unsigned long long> host((size_t)h->n_rep * 4);
+    std::vector<unsigned long long> host((size_t)h->n_rep * kActStride);
     CUDA_TRY(cudaMemcpyAsync(host.data(), h->d_act, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(cudaMemset2DAsync(h->d_act + 2, 4 * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][2..3]
+    CUDA_TRY(cudaMemset2DAsync(h->d_act + 2, kActStride * 8, 0, 2 * 8, (size_t)h->n_rep, h->stream));   // [rep][2..3]
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     for (int rep = 0; rep < h->n_rep; ++rep) {
-        evaluated_changed[rep * 2 + 0] = host[rep * 4 + 2];
-        evaluated_changed[rep * 2 + 1] = host[rep * 4 + 3];
+        evaluated_changed[rep * 2 + 0] = host[rep * kActStride + 2];
+        evaluated_changed[rep * 2 + 1] = host[rep * kActStride + 3];
     }
     return ISING3D_OK;
 }
@@ -1112,7 +1221,7 @@ int ising3d_get_state(ising3d_t *h, uint32_t *words, size_t n_words, uint64_t *s
     CUDA_TRY(cudaMemcpyAsync(words, h->state[h->cur], n_words * 4, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     if (sweep) *sweep = h->sweep;
-    return ISING3D_OK;
+    return probe_poll(h);
 }
 
 int ising3d_set_state(ising3d_t *h, const uint32_t *words, size_t n_words, uint64_t sweep)
@@ -1179,7 +1288,7 @@ int ising3d_sync(ising3d_t *h)
 {
     if (!h) return fail(ISING3D_EINVAL, "null handle");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    return ISING3D_OK;
+    return probe_poll(h);        // a probe of the AUTO policy that was in flight has landed: take its result
 }
 
 void ising3d_free(ising3d_t *h)
@@ -1188,6 +1297,8 @@ void ising3d_free(ising3d_t *h)
     cudaStreamSynchronize(h->stream);
     ising3d_release_radial(h);
     if (h->owns_mem && h->base) cudaFree(h->base);
+    if (h->h_probe) cudaFreeHost(h->h_probe);
+    if (h->probe_event) cudaEventDestroy(h->probe_event);
     delete h;
 }
 

@@ -143,7 +143,8 @@ constexpr int kActiveThreads = 256;
 constexpr int kActiveChunk = 2048;       // groups per work item: 64 flag words = 256 flag bytes, one per thread
 
 // ROLE = 0 / 1: first / second colour of the sweep (c = first ^ ROLE; keys.c1[ROLE] carries c).
-// stat[0] += groups evaluated, stat[1] += groups changed.
+// stat[0] += groups evaluated, stat[1] += groups changed, stat[2] += groups that held a site with
+// Delta E <= 0 when they were evaluated (what activity_flags_kernel counts, taken at the colour's update).
 // Work items (bricks of 2048 groups) are handed out through a ticket counter that is
 // never reset: this launch owns tickets base .. base + n_chunks - 1 (mod 2^32), and every CTA draws
 // exactly one ticket beyond them before it stops, so the next launch starts at
@@ -166,7 +167,7 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
     uint32_t *aw_own = awake + (size_t)c * (geo.G >> 5);
     uint32_t *aw_oth = awake + (size_t)(1 - c) * (geo.G >> 5);
     const uint32_t n_chunks = geo.G / kActiveChunk;
-    uint32_t evaluated = 0, changed = 0;
+    uint32_t evaluated = 0, changed = 0, held = 0;
     const uint8_t *flag_bytes = reinterpret_cast<const uint8_t *>(aw_own);
     // brick `chunk` = strip by (RB rows) of slab bz (PB planes); its groups are, plane by plane, RS
     // consecutive group indices from brick_base(chunk) + j * GP
@@ -229,6 +230,8 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
                 nw.w ^= e.tie.w & rho.w;
                 atomicOr(&keep[li >> 5], 1u << (li & 31));
             }
+            // a site with n >= 4 shows as det != s, one with n = 3 as a tie
+            if (anytie | (e.det.x ^ e.s.x) | (e.det.y ^ e.s.y) | (e.det.z ^ e.s.z) | (e.det.w ^ e.s.w)) ++held;
             const uint4 d = make_uint4(nw.x ^ e.s.x, nw.y ^ e.s.y, nw.z ^ e.s.z, nw.w ^ e.s.w);
             if (d.x | d.y | d.z | d.w) {
                 own[g] = nw;
@@ -252,10 +255,14 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
         }
         if (tid == 0) evaluated += total;
     }
-    for (int d = 16; d; d >>= 1) changed += __shfl_xor_sync(0xffffffffu, changed, d);
-    if (lane == 0 && (evaluated | changed)) {
+    for (int d = 16; d; d >>= 1) {
+        changed += __shfl_xor_sync(0xffffffffu, changed, d);
+        held += __shfl_xor_sync(0xffffffffu, held, d);
+    }
+    if (lane == 0 && (evaluated | changed | held)) {
         if (evaluated) atomicAdd(stat, (unsigned long long)evaluated);
         if (changed) atomicAdd(stat + 1, (unsigned long long)changed);
+        if (held) atomicAdd(stat + 2, (unsigned long long)held);
     }
 }
 
@@ -297,13 +304,26 @@ inline cudaError_t launch_active_sweep(uint32_t *state, uint32_t *awake, unsigne
     const ActiveGeom geo = make_active_geom(L);
     const SweepConsts keys = make_sweep_consts(seed, t, first);
     const uint32_t per_launch = geo.G / kActiveChunk + plan.grid;
+    // the host's ticket count follows the device counter only for launches that were accepted: after a
+    // refused launch the caller resets both (reset_active_tickets)
     active_halfsweep_kernel<0><<<plan.grid, kActiveThreads, 0, stream>>>(state, awake, first, stat, tickets,
                                                                        plan.next_ticket, geo, keys);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
     plan.next_ticket += per_launch;
     active_halfsweep_kernel<1><<<plan.grid, kActiveThreads, 0, stream>>>(state, awake, 1 - first, stat, tickets,
                                                                        plan.next_ticket, geo, keys);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
     plan.next_ticket += per_launch;
-    return cudaGetLastError();
+    return cudaSuccess;
+}
+
+// After a failed launch: device counter and host count back to zero, in stream order.
+inline cudaError_t reset_active_tickets(unsigned int *tickets, ActivePlan &plan, cudaStream_t stream)
+{
+    plan.next_ticket = 0;
+    return cudaMemsetAsync(tickets, 0, sizeof(unsigned int), stream);
 }
 
 }  // namespace ising

@@ -117,7 +117,10 @@ def test_active_sweep_against_oracle_L512_batch(B, orc):
 def test_auto_policy_switches_and_keeps_the_trajectory(B, orc):
     """AUTO at L = 512 with a short probe interval: a late-time-like state switches to the
     activity-driven kernel, an iid state stays on fused2, and either way the states equal the
-    oracle's; interleaving dense and activity-driven sweeps (flags rebuilt) changes nothing."""
+    oracle's; interleaving dense and activity-driven sweeps (flags rebuilt) changes nothing.
+    The probes do not block the host: a switch shows once the probe has landed, i.e. for certain
+    after a call that waits for the stream (sync, get_state); whether the sweeps queued in between
+    ran dense or activity-driven is a matter of timing and must not show in the state."""
     L = 512
     sim = B.Ising3D(L, [41])
     sim.set_activity_policy(4, 0.5, 0.9)
@@ -125,6 +128,7 @@ def test_auto_policy_switches_and_keeps_the_trajectory(B, orc):
     ref = orc.Oracle(L, 41)
     sim.sweep(9)                                   # iid start: probes at 4 and 8 see every group awake
     ref.sweep(9)
+    sim.sync()
     assert sim.variant_name == "fused2" and sim.last_activity > 0.9
     assert np.array_equal(sim.get_state(), ref.export_words())
     words = inputs.pack_spins(inputs.domain_spins(L, 11, block=32, p_minority=0.2, noise=0.0005))
@@ -132,15 +136,18 @@ def test_auto_policy_switches_and_keeps_the_trajectory(B, orc):
     ref.import_words(words, 200)
     assert sim.variant_name == "fused2"            # set_state voids the history
     sim.sweep(3)
-    assert sim.variant_name == "fused2"
-    sim.sweep(3)                                   # the probe after sweep 4 switches; 2 active sweeps follow
+    sim.sync()
+    assert sim.variant_name == "fused2"            # no probe yet
+    sim.sweep(1)                                   # the probe after sweep 4 ...
+    sim.sync()                                     # ... has landed now
     assert sim.variant_name == "active" and 0.0 < sim.last_activity < 0.5
+    sim.sweep(2)
     ref.sweep(6)
     assert np.array_equal(sim.get_state(), ref.export_words())
-    sim.sweep(11)
+    sim.sweep(11)                                  # tallies read after 4 and 8 active sweeps: still few groups
     ref.sweep(11)
-    assert sim.variant_name == "active"
     assert np.array_equal(sim.get_state(), ref.export_words())
+    assert sim.variant_name == "active" and 0.0 < sim.last_activity < 0.5
     # forced dense, then AUTO again (the flags are rebuilt at the next probe)
     sim.set_variant(B.VARIANT_FUSED2)
     sim.sweep(2)
@@ -148,14 +155,111 @@ def test_auto_policy_switches_and_keeps_the_trajectory(B, orc):
     assert sim.variant_name == "fused2"
     sim.sweep(7)
     ref.sweep(9)
-    assert sim.variant_name == "active"
     assert np.array_equal(sim.get_state(), ref.export_words())
+    assert sim.variant_name == "active"
     got, want = sim.measure(), ref.measure_full()
     assert int(got["n_up"][0]) == want["n_up"] and np.array_equal(got["antipar"][0], want["antipar"])
     # handing back: an iid state set into an active handle goes dense again
     sim.set_state(inputs.random_words(L, 1, 5), 0)
     sim.sweep(4)
+    sim.sync()
     assert sim.variant_name == "fused2"
+    sim.free()
+
+
+def test_auto_hands_back_when_activity_grows(B, orc):
+    """The way back, active -> fused2, taken by the policy itself (no set_state, no set_variant in
+    between): a 64^3 cube of up spins in a down sea starts with 8 groups that can change (its corners,
+    Delta E = 0) and erodes into ever more kinks -- 5e-5 of the groups after 4 sweeps, 1e-4 after 12,
+    3e-4 after 36 (counted with the oracle).  With on_below = 7e-5 and off_above = 2e-4 the handle
+    goes activity-driven at the first probe and must come back to fused2 by itself once the kernel's
+    own tally passes off_above; the trajectory is the oracle's throughout (eq. (6))."""
+    L = 512
+    words = inputs.pack_spins(inputs.cube(L, 100, 100, 100, 64))
+    sim = B.Ising3D(L, [9])
+    sim.set_activity_policy(4, 7e-5, 2e-4)
+    sim.set_state(words, 0)
+    seen, fracs, t = [], [], 0
+    for _ in range(24):
+        sim.sweep(4)
+        sim.sync()                     # the probe queued after these 4 sweeps has landed
+        t += 4
+        seen.append(sim.variant_name)
+        fracs.append(sim.last_activity)
+        if "active" in seen and seen[-2:] == ["fused2", "fused2"]:
+            break
+    assert seen[0] == "active", (seen, fracs)
+    first_back = seen.index("fused2")
+    assert first_back >= 2 and set(seen[:first_back]) == {"active"} and set(seen[first_back:]) == {"fused2"}, (seen, fracs)
+    assert fracs[first_back] > 2e-4 and all(0.0 < f <= 2e-4 for f in fracs[:first_back]), fracs
+    ev = sim.active_stats()[0]
+    assert ev[0] > 0 and ev[1] > 0      # the activity-driven kernel did run and did change groups
+    ref = orc.Oracle(L, 9, init=False)
+    ref.import_words(words, 0)
+    ref.sweep(t)
+    assert np.array_equal(sim.get_state(), ref.export_words())
+    assert list(sim.activity()[0][0]) == list(ref.activity())
+    sim.free()
+
+
+def test_auto_long_call_hands_over_on_its_own(B):
+    """One ising3d_sweep(5000) call under the default policy on a late-time state (config 4 at
+    t = 50 000, where under 11 % of the groups can change): nothing in the call waits for the GPU,
+    the probe result is picked up between launches, so the hand-over happens inside the call -- seen
+    in the launch count (two launches per activity-driven sweep, one per fused2 sweep) -- and the
+    state equals that of the same 5000 sweeps on fused2 alone."""
+    import torch
+    L, seed, t0, n = 1024, 3, 50_000, 5000
+    b = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED2)
+    b.sweep(t0)
+    nw = L ** 3 // 32
+    buf = torch.empty(nw, dtype=torch.int32, device="cuda")
+    b.get_state_device(buf.data_ptr(), nw)
+    a = B.Ising3D(L, [seed])
+    a.set_state_device(buf.data_ptr(), nw, t0)
+    assert a.variant_name == "fused2"
+    before = a.launch_count
+    a.sweep(n)
+    launches = a.launch_count - before
+    b.sweep(n)
+    assert launches > n + 1000, "the hand-over did not happen inside the call (%d launches)" % launches
+    assert np.array_equal(a.get_state(), b.get_state())
+    assert a.variant_name == "active" and 0.0 < a.last_activity < 0.11
+    a.free()
+    b.free()
+
+
+def test_default_handle_sweeps_can_be_stream_captured(B):
+    """ising3d_sweep under the default (AUTO) policy makes no synchronising call, so it can be
+    recorded into a CUDA graph: capture sweep(4) at sweep index t0 on a side stream, replay the graph
+    once, and the state equals that of a live sweep(4) from the same state and index (the sweep
+    index is a launch argument, so one replay is exactly sweeps t0 .. t0+3; an even count leaves the
+    ping-pong buffers where the handle believes them)."""
+    import torch
+    L, t0 = 512, 700
+    words = inputs.coarse_words(L, 31, block=16)
+    live = B.Ising3D(L, [77])
+    live.set_state(words, t0)
+    live.sweep(4)
+    want = live.get_state()
+    live.free()
+    side = torch.cuda.Stream()
+    sim = B.Ising3D(L, [77])
+    sim.set_activity_policy(2, 0.11, 0.14)      # a probe would fall inside the captured call
+    sim.sweep(2)                                # first use of the kernels (function attributes) outside the capture
+    sim.sync()
+    sim.set_stream(side.cuda_stream)
+    sim.set_state(words, t0)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side, capture_error_mode="thread_local"):
+        sim.sweep(4)
+    assert sim.sweep_count == t0 + 4
+    assert np.array_equal(sim.get_state(), words)      # recorded, not run
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(sim.get_state(), want)
+    sim.sweep(3)                                # and the handle goes on live, probes included
+    sim.sync()
     sim.free()
 
 
@@ -222,6 +326,7 @@ def test_auto_run_equals_fused2_run_config4(B):
     b = B.Ising3D(L, [seed], variant=B.VARIANT_FUSED2)
     a.sweep(n)
     b.sweep(n)
+    a.sync()
     assert a.variant_name == "active" and b.variant_name == "fused2"
     assert 0.0 < a.last_activity < 0.11
     ev = a.active_stats()[0]
@@ -246,8 +351,8 @@ def test_auto_policy_batch_of_two(B, orc):
     for r, ww in zip(refs, w):
         r.import_words(ww, 40)
     sim.sweep(8)
-    assert sim.variant_name == "active"
     got = sim.get_state().reshape(2, -1)
+    assert sim.variant_name == "active"
     for i, r in enumerate(refs):
         r.sweep(8)
         assert np.array_equal(got[i], r.export_words()), "replica %d" % i
