@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--L", type=int, default=2048)
     ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (throughput window)")
-    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2", "fused3"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "generic", "fused", "fused2"])
     ap.add_argument("--ref-L", type=int, default=512, help="--impl reference: lattice size of the CPU sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -266,8 +266,7 @@ def run_ours(args):
     L, S = args.L, args.sweeps
     seed = rank_seed(rank)
     variant = {"auto": binding.VARIANT_AUTO, "generic": binding.VARIANT_GENERIC,
-               "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2,
-               "fused3": binding.VARIANT_FUSED3}[args.variant]
+               "fused": binding.VARIANT_FUSED, "fused2": binding.VARIANT_FUSED2}[args.variant]
     sim = binding.Ising3D(L, [seed], variant=variant)
     N = L ** 3
     n_words = N // 32
@@ -394,10 +393,8 @@ def run_ours(args):
 
     # ---------------- roofline of the dominant kernel (the sweep kernel) ----------------
     peak, peak_src, peaks = measured_peak()
-    kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel",
-              "fused3": "fused3_sweep2_kernel"}.get(timed_kernel, "halfsweep_generic_kernel")
-    # fused3: one launch = two sweeps (an odd last sweep of a step runs on fused2; S is even here)
-    launches_per_sweep = {"fused": 1, "fused2": 1, "fused3": 0.5}.get(timed_kernel, 2)
+    kernel = {"fused": "fused_sweep_kernel", "fused2": "fused2_sweep_kernel"}.get(timed_kernel, "halfsweep_generic_kernel")
+    launches_per_sweep = {"fused": 1, "fused2": 1}.get(timed_kernel, 2)
     avg_launch_ms = sweep_ms / (S * launches_per_sweep)
     algo_bytes_per_launch = ALGO_BYTES_PER_SITE_UPDATE * N / launches_per_sweep
     achieved = algo_bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9

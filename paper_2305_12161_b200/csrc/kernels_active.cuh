@@ -14,8 +14,10 @@
 // active_halfsweep_kernel keeps it: it evaluates the flagged groups of colour c only, in place
 // (same-colour sites do not interact, so the order is free), leaves a group's flag
 // set iff the group still holds a tie (n = 3: the next sweep's random bit can flip it; a site with
-// n >= 4 has flipped and now has n <= 2), and sets the flag of every other-colour group that reads
-// a word it changed (same group index, y+-1, z+-1, and the row neighbour that takes the edge bit).
+// n >= 4 has flipped and now has n <= 2), and sets the flag of the other-colour groups that read
+// a word it changed (same group index, y+-1, z+-1, and the row neighbour that takes the edge bit) -- of
+// those only that hold a neighbour of a flipped site which now differs from it: that neighbour's n went
+// up, any other neighbour's n went down, and a sleeping group's sites all have n <= 2.
 // The random bits are the same counter-based Philox4x32-10 bits (q, t, colour, 0) as everywhere
 // (D5), drawn only for groups that hold a tie, so the trajectory is bit-identical to the dense
 // kernels'.
@@ -139,6 +141,21 @@ activity_flags_kernel(const uint32_t *__restrict__ state, uint32_t *__restrict__
     if (threadIdx.x == 0 && cta_count) atomicAdd(count + c, (unsigned long long)cta_count);
 }
 
+// A second read of words eval_group has just read (they sit in L1).  volatile: the compiler must not merge
+// it with the first read and keep 21 more registers alive across the Philox call for a branch few groups take.
+__device__ __forceinline__ uint4 ldg_again(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ldg_again(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 constexpr int kActiveThreads = 256;
 constexpr int kActiveChunk = 2048;       // groups per work item: 64 flag words = 256 flag bytes, one per thread
 
@@ -149,8 +166,10 @@ constexpr int kActiveChunk = 2048;       // groups per work item: 64 flag words 
 // never reset: this launch owns tickets base .. base + n_chunks - 1 (mod 2^32), and every CTA draws
 // exactly one ticket beyond them before it stops, so the next launch starts at
 // base + n_chunks + gridDim.x (the host keeps count).
+// Four CTAs per SM (64 registers, no spills; ptxas takes 80 unasked, which leaves room for three): the kernel
+// waits for scattered sectors, so resident warps are what it needs (two CTAs per SM: 60 % slower).
 template <int ROLE>
-__global__ void __launch_bounds__(kActiveThreads)
+__global__ void __launch_bounds__(kActiveThreads, 4)
 active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awake, const int c,
                         unsigned long long *__restrict__ stat, unsigned int *__restrict__ tickets,
                         const uint32_t base_ticket, const ActiveGeom geo,
@@ -236,16 +255,34 @@ active_halfsweep_kernel(uint32_t *__restrict__ state, uint32_t *__restrict__ awa
             if (d.x | d.y | d.z | d.w) {
                 own[g] = nw;
                 ++changed;
-                // wake the other-colour groups that read the changed words (D4)
-                atomicOr(aw_oth + (g >> 5), 1u << (g & 31));
-                atomicOr(aw_oth + (n.gyp >> 5), 1u << (n.gyp & 31));
-                atomicOr(aw_oth + (n.gym >> 5), 1u << (n.gym & 31));
-                atomicOr(aw_oth + (n.gzp >> 5), 1u << (n.gzp & 31));
-                atomicOr(aw_oth + (n.gzm >> 5), 1u << (n.gzm & 31));
-                // the other colour's in-row direction in this row is 1 - o: with o = 1 its group x4+1
-                // takes our bit 127, with o = 0 its group x4-1 takes our bit 0
-                if (n.o == 1 && (d.w >> 31)) atomicOr(aw_oth + (n.gnext >> 5), 1u << (n.gnext & 31));
-                if (n.o == 0 && (d.x & 1u)) atomicOr(aw_oth + (n.gprev >> 5), 1u << (n.gprev & 31));
+                // Wake other-colour groups (D4).  A flip moves the antiparallel count n of each of its six
+                // neighbours by one: up if the neighbour differs from the new spin, down if it equals it.  A
+                // sleeping group has n <= 2 on all its sites, and only a step up can bring one to n >= 3,
+                // so a group is woken only if it holds a neighbour, of a flipped site, that differs from the
+                // new spin.  The neighbour words are the ones eval_group just read (L1).
+                auto up = [&](const uint4 &v) -> uint32_t {
+                    return (d.x & (nw.x ^ v.x)) | (d.y & (nw.y ^ v.y)) | (d.z & (nw.z ^ v.z)) | (d.w & (nw.w ^ v.w));
+                };
+                // one neighbour word at a time (few registers live): y+-1, z+-1
+                if (up(ldg_again(oth + n.gyp))) atomicOr(aw_oth + (n.gyp >> 5), 1u << (n.gyp & 31));
+                if (up(ldg_again(oth + n.gym))) atomicOr(aw_oth + (n.gym >> 5), 1u << (n.gym & 31));
+                if (up(ldg_again(oth + n.gzp))) atomicOr(aw_oth + (n.gzp >> 5), 1u << (n.gzp & 31));
+                if (up(ldg_again(oth + n.gzm))) atomicOr(aw_oth + (n.gzm >> 5), 1u << (n.gzm & 31));
+                // in-row neighbours: bit k of the same-index group and the bit beside it; the one bit of x
+                // that came from `edge` (bit 127 with o = 1, bit 0 with o = 0) lies in the next / previous group
+                const uint4 a = ldg_again(oth + g);
+                const uint32_t *othw = reinterpret_cast<const uint32_t *>(oth);
+                const uint32_t edge = ldg_again(othw + (n.o ? 4 * (size_t)n.gnext : 4 * (size_t)n.gprev + 3));
+                const uint4 x = xshift(a, n.o, edge);
+                uint4 ux = make_uint4(d.x & (nw.x ^ x.x), d.y & (nw.y ^ x.y), d.z & (nw.z ^ x.z), d.w & (nw.w ^ x.w));
+                const uint32_t up_edge = n.o ? (ux.w >> 31) : (ux.x & 1u);
+                if (n.o) ux.w &= 0x7fffffffu;
+                else ux.x &= ~1u;
+                if (up(a) | ux.x | ux.y | ux.z | ux.w) atomicOr(aw_oth + (g >> 5), 1u << (g & 31));
+                if (up_edge) {
+                    const uint32_t ge = n.o ? n.gnext : n.gprev;
+                    atomicOr(aw_oth + (ge >> 5), 1u << (ge & 31));
+                }
             }
         }
         __syncthreads();

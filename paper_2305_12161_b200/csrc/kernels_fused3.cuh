@@ -1,3 +1,9 @@
+// EXPERIMENT, FROZEN.  Kept as the evidence that the sweep is bound by the SM, not by HBM (half the DRAM
+// traffic per sweep, no gain in time: profiles/r1g_fused3_full.md).  Opt-in only
+// (ISING3D_VARIANT_FUSED3), oracle-tested as it stands, but not developed further: later work on fused2
+// (instruction trims, double checkerboard, L = 1536, activity hand-over) was not brought over, and
+// bench.py no longer offers it.
+//
 // Two sweeps per launch (temporal blocking of a2+a3+a4), L in {1024, 2048}, cycle 01.
 //
 // kernels_fused2.cuh moves N/4 bytes per sweep and sits between its memory time and its compute

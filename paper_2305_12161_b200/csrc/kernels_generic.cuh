@@ -176,142 +176,28 @@ struct GlauberTables {
 // T = f(c2, c1, c0) word by word with the truth table `lut` (bit n = value for n = 4 c2 + 2 c1 + c0):
 // one LOP3 per word whose immediate is the table, reached through a 128-entry jump table (brx.idx;
 // the C++ switch is lowered to a seven-level compare tree instead, 14 instructions per dispatch).
+// The 128 cases differ only in the immediate, so the preprocessor writes them: case 0xHL has the label
+// GLHL and the immediate 0xHL (H = 0..7, L = 0..f).
+#define ISING_GL_LBL(h, l) "GL" #h #l
+#define ISING_GL_TGT(h, l) ISING_GL_LBL(h, l) ", "
+#define ISING_GL_CASE(h, l)                                                                                    \
+    ISING_GL_LBL(h, l) ": lop3.b32 %0, %4, %8, %13, 0x" #h #l "; lop3.b32 %1, %5, %9, %14, 0x" #h #l             \
+                       "; lop3.b32 %2, %6, %10, %15, 0x" #h #l "; lop3.b32 %3, %7, %11, %16, 0x" #h #l "; bra.uni GLE;\n"
+#define ISING_GL_ROW(M, h)                                                                                     \
+    M(h, 0) M(h, 1) M(h, 2) M(h, 3) M(h, 4) M(h, 5) M(h, 6) M(h, 7) M(h, 8) M(h, 9) M(h, a) M(h, b) M(h, c) M(h, d) M(h, e) M(h, f)
+#define ISING_GL_ALL(M)                                                                                        \
+    ISING_GL_ROW(M, 0) ISING_GL_ROW(M, 1) ISING_GL_ROW(M, 2) ISING_GL_ROW(M, 3) ISING_GL_ROW(M, 4) ISING_GL_ROW(M, 5)  \
+    ISING_GL_ROW(M, 6) ISING_GL_ROW(M, 7)
 __device__ __forceinline__ uint4 class_select(const uint32_t lut, const uint4 c2, const uint4 c1, const uint4 c0)
 {
     uint4 T;
     const uint32_t idx = lut & 127u;
     asm volatile(
         "{\n"
-        "GLT: .branchtargets GL0, GL1, GL2, GL3, GL4, GL5, GL6, GL7, GL8, GL9, GL10, GL11, GL12, GL13, GL14, GL15, GL16, GL17, GL18, GL19, GL20, GL21, GL22, GL23, GL24, GL25, GL26, GL27, GL28, GL29, GL30, GL31, GL32, GL33, GL34, GL35, GL36, GL37, GL38, GL39, GL40, GL41, GL42, GL43, GL44, GL45, GL46, GL47, GL48, GL49, GL50, GL51, GL52, GL53, GL54, GL55, GL56, GL57, GL58, GL59, GL60, GL61, GL62, GL63, GL64, GL65, GL66, GL67, GL68, GL69, GL70, GL71, GL72, GL73, GL74, GL75, GL76, GL77, GL78, GL79, GL80, GL81, GL82, GL83, GL84, GL85, GL86, GL87, GL88, GL89, GL90, GL91, GL92, GL93, GL94, GL95, GL96, GL97, GL98, GL99, GL100, GL101, GL102, GL103, GL104, GL105, GL106, GL107, GL108, GL109, GL110, GL111, GL112, GL113, GL114, GL115, GL116, GL117, GL118, GL119, GL120, GL121, GL122, GL123, GL124, GL125, GL126, GL127;\n"
+        // targets 0..127 in index order; GLE closes the list and is never indexed (idx < 128)
+        "GLT: .branchtargets " ISING_GL_ALL(ISING_GL_TGT) "GLE;\n"
         "brx.idx %12, GLT;\n"
-        "GL0: lop3.b32 %0, %4, %8, %13, 0; lop3.b32 %1, %5, %9, %14, 0; lop3.b32 %2, %6, %10, %15, 0; lop3.b32 %3, %7, %11, %16, 0; bra.uni GLE;\n"
-        "GL1: lop3.b32 %0, %4, %8, %13, 1; lop3.b32 %1, %5, %9, %14, 1; lop3.b32 %2, %6, %10, %15, 1; lop3.b32 %3, %7, %11, %16, 1; bra.uni GLE;\n"
-        "GL2: lop3.b32 %0, %4, %8, %13, 2; lop3.b32 %1, %5, %9, %14, 2; lop3.b32 %2, %6, %10, %15, 2; lop3.b32 %3, %7, %11, %16, 2; bra.uni GLE;\n"
-        "GL3: lop3.b32 %0, %4, %8, %13, 3; lop3.b32 %1, %5, %9, %14, 3; lop3.b32 %2, %6, %10, %15, 3; lop3.b32 %3, %7, %11, %16, 3; bra.uni GLE;\n"
-        "GL4: lop3.b32 %0, %4, %8, %13, 4; lop3.b32 %1, %5, %9, %14, 4; lop3.b32 %2, %6, %10, %15, 4; lop3.b32 %3, %7, %11, %16, 4; bra.uni GLE;\n"
-        "GL5: lop3.b32 %0, %4, %8, %13, 5; lop3.b32 %1, %5, %9, %14, 5; lop3.b32 %2, %6, %10, %15, 5; lop3.b32 %3, %7, %11, %16, 5; bra.uni GLE;\n"
-        "GL6: lop3.b32 %0, %4, %8, %13, 6; lop3.b32 %1, %5, %9, %14, 6; lop3.b32 %2, %6, %10, %15, 6; lop3.b32 %3, %7, %11, %16, 6; bra.uni GLE;\n"
-        "GL7: lop3.b32 %0, %4, %8, %13, 7; lop3.b32 %1, %5, %9, %14, 7; lop3.b32 %2, %6, %10, %15, 7; lop3.b32 %3, %7, %11, %16, 7; bra.uni GLE;\n"
-        "GL8: lop3.b32 %0, %4, %8, %13, 8; lop3.b32 %1, %5, %9, %14, 8; lop3.b32 %2, %6, %10, %15, 8; lop3.b32 %3, %7, %11, %16, 8; bra.uni GLE;\n"
-        "GL9: lop3.b32 %0, %4, %8, %13, 9; lop3.b32 %1, %5, %9, %14, 9; lop3.b32 %2, %6, %10, %15, 9; lop3.b32 %3, %7, %11, %16, 9; bra.uni GLE;\n"
-        "GL10: lop3.b32 %0, %4, %8, %13, 10; lop3.b32 %1, %5, %9, %14, 10; lop3.b32 %2, %6, %10, %15, 10; lop3.b32 %3, %7, %11, %16, 10; bra.uni GLE;\n"
-        "GL11: lop3.b32 %0, %4, %8, %13, 11; lop3.b32 %1, %5, %9, %14, 11; lop3.b32 %2, %6, %10, %15, 11; lop3.b32 %3, %7, %11, %16, 11; bra.uni GLE;\n"
-        "GL12: lop3.b32 %0, %4, %8, %13, 12; lop3.b32 %1, %5, %9, %14, 12; lop3.b32 %2, %6, %10, %15, 12; lop3.b32 %3, %7, %11, %16, 12; bra.uni GLE;\n"
-        "GL13: lop3.b32 %0, %4, %8, %13, 13; lop3.b32 %1, %5, %9, %14, 13; lop3.b32 %2, %6, %10, %15, 13; lop3.b32 %3, %7, %11, %16, 13; bra.uni GLE;\n"
-        "GL14: lop3.b32 %0, %4, %8, %13, 14; lop3.b32 %1, %5, %9, %14, 14; lop3.b32 %2, %6, %10, %15, 14; lop3.b32 %3, %7, %11, %16, 14; bra.uni GLE;\n"
-        "GL15: lop3.b32 %0, %4, %8, %13, 15; lop3.b32 %1, %5, %9, %14, 15; lop3.b32 %2, %6, %10, %15, 15; lop3.b32 %3, %7, %11, %16, 15; bra.uni GLE;\n"
-        "GL16: lop3.b32 %0, %4, %8, %13, 16; lop3.b32 %1, %5, %9, %14, 16; lop3.b32 %2, %6, %10, %15, 16; lop3.b32 %3, %7, %11, %16, 16; bra.uni GLE;\n"
-        "GL17: lop3.b32 %0, %4, %8, %13, 17; lop3.b32 %1, %5, %9, %14, 17; lop3.b32 %2, %6, %10, %15, 17; lop3.b32 %3, %7, %11, %16, 17; bra.uni GLE;\n"
-        "GL18: lop3.b32 %0, %4, %8, %13, 18; lop3.b32 %1, %5, %9, %14, 18; lop3.b32 %2, %6, %10, %15, 18; lop3.b32 %3, %7, %11, %16, 18; bra.uni GLE;\n"
-        "GL19: lop3.b32 %0, %4, %8, %13, 19; lop3.b32 %1, %5, %9, %14, 19; lop3.b32 %2, %6, %10, %15, 19; lop3.b32 %3, %7, %11, %16, 19; bra.uni GLE;\n"
-        "GL20: lop3.b32 %0, %4, %8, %13, 20; lop3.b32 %1, %5, %9, %14, 20; lop3.b32 %2, %6, %10, %15, 20; lop3.b32 %3, %7, %11, %16, 20; bra.uni GLE;\n"
-        "GL21: lop3.b32 %0, %4, %8, %13, 21; lop3.b32 %1, %5, %9, %14, 21; lop3.b32 %2, %6, %10, %15, 21; lop3.b32 %3, %7, %11, %16, 21; bra.uni GLE;\n"
-        "GL22: lop3.b32 %0, %4, %8, %13, 22; lop3.b32 %1, %5, %9, %14, 22; lop3.b32 %2, %6, %10, %15, 22; lop3.b32 %3, %7, %11, %16, 22; bra.uni GLE;\n"
-        "GL23: lop3.b32 %0, %4, %8, %13, 23; lop3.b32 %1, %5, %9, %14, 23; lop3.b32 %2, %6, %10, %15, 23; lop3.b32 %3, %7, %11, %16, 23; bra.uni GLE;\n"
-        "GL24: lop3.b32 %0, %4, %8, %13, 24; lop3.b32 %1, %5, %9, %14, 24; lop3.b32 %2, %6, %10, %15, 24; lop3.b32 %3, %7, %11, %16, 24; bra.uni GLE;\n"
-        "GL25: lop3.b32 %0, %4, %8, %13, 25; lop3.b32 %1, %5, %9, %14, 25; lop3.b32 %2, %6, %10, %15, 25; lop3.b32 %3, %7, %11, %16, 25; bra.uni GLE;\n"
-        "GL26: lop3.b32 %0, %4, %8, %13, 26; lop3.b32 %1, %5, %9, %14, 26; lop3.b32 %2, %6, %10, %15, 26; lop3.b32 %3, %7, %11, %16, 26; bra.uni GLE;\n"
-        "GL27: lop3.b32 %0, %4, %8, %13, 27; lop3.b32 %1, %5, %9, %14, 27; lop3.b32 %2, %6, %10, %15, 27; lop3.b32 %3, %7, %11, %16, 27; bra.uni GLE;\n"
-        "GL28: lop3.b32 %0, %4, %8, %13, 28; lop3.b32 %1, %5, %9, %14, 28; lop3.b32 %2, %6, %10, %15, 28; lop3.b32 %3, %7, %11, %16, 28; bra.uni GLE;\n"
-        "GL29: lop3.b32 %0, %4, %8, %13, 29; lop3.b32 %1, %5, %9, %14, 29; lop3.b32 %2, %6, %10, %15, 29; lop3.b32 %3, %7, %11, %16, 29; bra.uni GLE;\n"
-        "GL30: lop3.b32 %0, %4, %8, %13, 30; lop3.b32 %1, %5, %9, %14, 30; lop3.b32 %2, %6, %10, %15, 30; lop3.b32 %3, %7, %11, %16, 30; bra.uni GLE;\n"
-        "GL31: lop3.b32 %0, %4, %8, %13, 31; lop3.b32 %1, %5, %9, %14, 31; lop3.b32 %2, %6, %10, %15, 31; lop3.b32 %3, %7, %11, %16, 31; bra.uni GLE;\n"
-        "GL32: lop3.b32 %0, %4, %8, %13, 32; lop3.b32 %1, %5, %9, %14, 32; lop3.b32 %2, %6, %10, %15, 32; lop3.b32 %3, %7, %11, %16, 32; bra.uni GLE;\n"
-        "GL33: lop3.b32 %0, %4, %8, %13, 33; lop3.b32 %1, %5, %9, %14, 33; lop3.b32 %2, %6, %10, %15, 33; lop3.b32 %3, %7, %11, %16, 33; bra.uni GLE;\n"
-        "GL34: lop3.b32 %0, %4, %8, %13, 34; lop3.b32 %1, %5, %9, %14, 34; lop3.b32 %2, %6, %10, %15, 34; lop3.b32 %3, %7, %11, %16, 34; bra.uni GLE;\n"
-        "GL35: lop3.b32 %0, %4, %8, %13, 35; lop3.b32 %1, %5, %9, %14, 35; lop3.b32 %2, %6, %10, %15, 35; lop3.b32 %3, %7, %11, %16, 35; bra.uni GLE;\n"
-        "GL36: lop3.b32 %0, %4, %8, %13, 36; lop3.b32 %1, %5, %9, %14, 36; lop3.b32 %2, %6, %10, %15, 36; lop3.b32 %3, %7, %11, %16, 36; bra.uni GLE;\n"
-        "GL37: lop3.b32 %0, %4, %8, %13, 37; lop3.b32 %1, %5, %9, %14, 37; lop3.b32 %2, %6, %10, %15, 37; lop3.b32 %3, %7, %11, %16, 37; bra.uni GLE;\n"
-        "GL38: lop3.b32 %0, %4, %8, %13, 38; lop3.b32 %1, %5, %9, %14, 38; lop3.b32 %2, %6, %10, %15, 38; lop3.b32 %3, %7, %11, %16, 38; bra.uni GLE;\n"
-        "GL39: lop3.b32 %0, %4, %8, %13, 39; lop3.b32 %1, %5, %9, %14, 39; lop3.b32 %2, %6, %10, %15, 39; lop3.b32 %3, %7, %11, %16, 39; bra.uni GLE;\n"
-        "GL40: lop3.b32 %0, %4, %8, %13, 40; lop3.b32 %1, %5, %9, %14, 40; lop3.b32 %2, %6, %10, %15, 40; lop3.b32 %3, %7, %11, %16, 40; bra.uni GLE;\n"
-        "GL41: lop3.b32 %0, %4, %8, %13, 41; lop3.b32 %1, %5, %9, %14, 41; lop3.b32 %2, %6, %10, %15, 41; lop3.b32 %3, %7, %11, %16, 41; bra.uni GLE;\n"
-        "GL42: lop3.b32 %0, %4, %8, %13, 42; lop3.b32 %1, %5, %9, %14, 42; lop3.b32 %2, %6, %10, %15, 42; lop3.b32 %3, %7, %11, %16, 42; bra.uni GLE;\n"
-        "GL43: lop3.b32 %0, %4, %8, %13, 43; lop3.b32 %1, %5, %9, %14, 43; lop3.b32 %2, %6, %10, %15, 43; lop3.b32 %3, %7, %11, %16, 43; bra.uni GLE;\n"
-        "GL44: lop3.b32 %0, %4, %8, %13, 44; lop3.b32 %1, %5, %9, %14, 44; lop3.b32 %2, %6, %10, %15, 44; lop3.b32 %3, %7, %11, %16, 44; bra.uni GLE;\n"
-        "GL45: lop3.b32 %0, %4, %8, %13, 45; lop3.b32 %1, %5, %9, %14, 45; lop3.b32 %2, %6, %10, %15, 45; lop3.b32 %3, %7, %11, %16, 45; bra.uni GLE;\n"
-        "GL46: lop3.b32 %0, %4, %8, %13, 46; lop3.b32 %1, %5, %9, %14, 46; lop3.b32 %2, %6, %10, %15, 46; lop3.b32 %3, %7, %11, %16, 46; bra.uni GLE;\n"
-        "GL47: lop3.b32 %0, %4, %8, %13, 47; lop3.b32 %1, %5, %9, %14, 47; lop3.b32 %2, %6, %10, %15, 47; lop3.b32 %3, %7, %11, %16, 47; bra.uni GLE;\n"
-        "GL48: lop3.b32 %0, %4, %8, %13, 48; lop3.b32 %1, %5, %9, %14, 48; lop3.b32 %2, %6, %10, %15, 48; lop3.b32 %3, %7, %11, %16, 48; bra.uni GLE;\n"
-        "GL49: lop3.b32 %0, %4, %8, %13, 49; lop3.b32 %1, %5, %9, %14, 49; lop3.b32 %2, %6, %10, %15, 49; lop3.b32 %3, %7, %11, %16, 49; bra.uni GLE;\n"
-        "GL50: lop3.b32 %0, %4, %8, %13, 50; lop3.b32 %1, %5, %9, %14, 50; lop3.b32 %2, %6, %10, %15, 50; lop3.b32 %3, %7, %11, %16, 50; bra.uni GLE;\n"
-        "GL51: lop3.b32 %0, %4, %8, %13, 51; lop3.b32 %1, %5, %9, %14, 51; lop3.b32 %2, %6, %10, %15, 51; lop3.b32 %3, %7, %11, %16, 51; bra.uni GLE;\n"
-        "GL52: lop3.b32 %0, %4, %8, %13, 52; lop3.b32 %1, %5, %9, %14, 52; lop3.b32 %2, %6, %10, %15, 52; lop3.b32 %3, %7, %11, %16, 52; bra.uni GLE;\n"
-        "GL53: lop3.b32 %0, %4, %8, %13, 53; lop3.b32 %1, %5, %9, %14, 53; lop3.b32 %2, %6, %10, %15, 53; lop3.b32 %3, %7, %11, %16, 53; bra.uni GLE;\n"
-        "GL54: lop3.b32 %0, %4, %8, %13, 54; lop3.b32 %1, %5, %9, %14, 54; lop3.b32 %2, %6, %10, %15, 54; lop3.b32 %3, %7, %11, %16, 54; bra.uni GLE;\n"
-        "GL55: lop3.b32 %0, %4, %8, %13, 55; lop3.b32 %1, %5, %9, %14, 55; lop3.b32 %2, %6, %10, %15, 55; lop3.b32 %3, %7, %11, %16, 55; bra.uni GLE;\n"
-        "GL56: lop3.b32 %0, %4, %8, %13, 56; lop3.b32 %1, %5, %9, %14, 56; lop3.b32 %2, %6, %10, %15, 56; lop3.b32 %3, %7, %11, %16, 56; bra.uni GLE;\n"
-        "GL57: lop3.b32 %0, %4, %8, %13, 57; lop3.b32 %1, %5, %9, %14, 57; lop3.b32 %2, %6, %10, %15, 57; lop3.b32 %3, %7, %11, %16, 57; bra.uni GLE;\n"
-        "GL58: lop3.b32 %0, %4, %8, %13, 58; lop3.b32 %1, %5, %9, %14, 58; lop3.b32 %2, %6, %10, %15, 58; lop3.b32 %3, %7, %11, %16, 58; bra.uni GLE;\n"
-        "GL59: lop3.b32 %0, %4, %8, %13, 59; lop3.b32 %1, %5, %9, %14, 59; lop3.b32 %2, %6, %10, %15, 59; lop3.b32 %3, %7, %11, %16, 59; bra.uni GLE;\n"
-        "GL60: lop3.b32 %0, %4, %8, %13, 60; lop3.b32 %1, %5, %9, %14, 60; lop3.b32 %2, %6, %10, %15, 60; lop3.b32 %3, %7, %11, %16, 60; bra.uni GLE;\n"
-        "GL61: lop3.b32 %0, %4, %8, %13, 61; lop3.b32 %1, %5, %9, %14, 61; lop3.b32 %2, %6, %10, %15, 61; lop3.b32 %3, %7, %11, %16, 61; bra.uni GLE;\n"
-        "GL62: lop3.b32 %0, %4, %8, %13, 62; lop3.b32 %1, %5, %9, %14, 62; lop3.b32 %2, %6, %10, %15, 62; lop3.b32 %3, %7, %11, %16, 62; bra.uni GLE;\n"
-        "GL63: lop3.b32 %0, %4, %8, %13, 63; lop3.b32 %1, %5, %9, %14, 63; lop3.b32 %2, %6, %10, %15, 63; lop3.b32 %3, %7, %11, %16, 63; bra.uni GLE;\n"
-        "GL64: lop3.b32 %0, %4, %8, %13, 64; lop3.b32 %1, %5, %9, %14, 64; lop3.b32 %2, %6, %10, %15, 64; lop3.b32 %3, %7, %11, %16, 64; bra.uni GLE;\n"
-        "GL65: lop3.b32 %0, %4, %8, %13, 65; lop3.b32 %1, %5, %9, %14, 65; lop3.b32 %2, %6, %10, %15, 65; lop3.b32 %3, %7, %11, %16, 65; bra.uni GLE;\n"
-        "GL66: lop3.b32 %0, %4, %8, %13, 66; lop3.b32 %1, %5, %9, %14, 66; lop3.b32 %2, %6, %10, %15, 66; lop3.b32 %3, %7, %11, %16, 66; bra.uni GLE;\n"
-        "GL67: lop3.b32 %0, %4, %8, %13, 67; lop3.b32 %1, %5, %9, %14, 67; lop3.b32 %2, %6, %10, %15, 67; lop3.b32 %3, %7, %11, %16, 67; bra.uni GLE;\n"
-        "GL68: lop3.b32 %0, %4, %8, %13, 68; lop3.b32 %1, %5, %9, %14, 68; lop3.b32 %2, %6, %10, %15, 68; lop3.b32 %3, %7, %11, %16, 68; bra.uni GLE;\n"
-        "GL69: lop3.b32 %0, %4, %8, %13, 69; lop3.b32 %1, %5, %9, %14, 69; lop3.b32 %2, %6, %10, %15, 69; lop3.b32 %3, %7, %11, %16, 69; bra.uni GLE;\n"
-        "GL70: lop3.b32 %0, %4, %8, %13, 70; lop3.b32 %1, %5, %9, %14, 70; lop3.b32 %2, %6, %10, %15, 70; lop3.b32 %3, %7, %11, %16, 70; bra.uni GLE;\n"
-        "GL71: lop3.b32 %0, %4, %8, %13, 71; lop3.b32 %1, %5, %9, %14, 71; lop3.b32 %2, %6, %10, %15, 71; lop3.b32 %3, %7, %11, %16, 71; bra.uni GLE;\n"
-        "GL72: lop3.b32 %0, %4, %8, %13, 72; lop3.b32 %1, %5, %9, %14, 72; lop3.b32 %2, %6, %10, %15, 72; lop3.b32 %3, %7, %11, %16, 72; bra.uni GLE;\n"
-        "GL73: lop3.b32 %0, %4, %8, %13, 73; lop3.b32 %1, %5, %9, %14, 73; lop3.b32 %2, %6, %10, %15, 73; lop3.b32 %3, %7, %11, %16, 73; bra.uni GLE;\n"
-        "GL74: lop3.b32 %0, %4, %8, %13, 74; lop3.b32 %1, %5, %9, %14, 74; lop3.b32 %2, %6, %10, %15, 74; lop3.b32 %3, %7, %11, %16, 74; bra.uni GLE;\n"
-        "GL75: lop3.b32 %0, %4, %8, %13, 75; lop3.b32 %1, %5, %9, %14, 75; lop3.b32 %2, %6, %10, %15, 75; lop3.b32 %3, %7, %11, %16, 75; bra.uni GLE;\n"
-        "GL76: lop3.b32 %0, %4, %8, %13, 76; lop3.b32 %1, %5, %9, %14, 76; lop3.b32 %2, %6, %10, %15, 76; lop3.b32 %3, %7, %11, %16, 76; bra.uni GLE;\n"
-        "GL77: lop3.b32 %0, %4, %8, %13, 77; lop3.b32 %1, %5, %9, %14, 77; lop3.b32 %2, %6, %10, %15, 77; lop3.b32 %3, %7, %11, %16, 77; bra.uni GLE;\n"
-        "GL78: lop3.b32 %0, %4, %8, %13, 78; lop3.b32 %1, %5, %9, %14, 78; lop3.b32 %2, %6, %10, %15, 78; lop3.b32 %3, %7, %11, %16, 78; bra.uni GLE;\n"
-        "GL79: lop3.b32 %0, %4, %8, %13, 79; lop3.b32 %1, %5, %9, %14, 79; lop3.b32 %2, %6, %10, %15, 79; lop3.b32 %3, %7, %11, %16, 79; bra.uni GLE;\n"
-        "GL80: lop3.b32 %0, %4, %8, %13, 80; lop3.b32 %1, %5, %9, %14, 80; lop3.b32 %2, %6, %10, %15, 80; lop3.b32 %3, %7, %11, %16, 80; bra.uni GLE;\n"
-        "GL81: lop3.b32 %0, %4, %8, %13, 81; lop3.b32 %1, %5, %9, %14, 81; lop3.b32 %2, %6, %10, %15, 81; lop3.b32 %3, %7, %11, %16, 81; bra.uni GLE;\n"
-        "GL82: lop3.b32 %0, %4, %8, %13, 82; lop3.b32 %1, %5, %9, %14, 82; lop3.b32 %2, %6, %10, %15, 82; lop3.b32 %3, %7, %11, %16, 82; bra.uni GLE;\n"
-        "GL83: lop3.b32 %0, %4, %8, %13, 83; lop3.b32 %1, %5, %9, %14, 83; lop3.b32 %2, %6, %10, %15, 83; lop3.b32 %3, %7, %11, %16, 83; bra.uni GLE;\n"
-        "GL84: lop3.b32 %0, %4, %8, %13, 84; lop3.b32 %1, %5, %9, %14, 84; lop3.b32 %2, %6, %10, %15, 84; lop3.b32 %3, %7, %11, %16, 84; bra.uni GLE;\n"
-        "GL85: lop3.b32 %0, %4, %8, %13, 85; lop3.b32 %1, %5, %9, %14, 85; lop3.b32 %2, %6, %10, %15, 85; lop3.b32 %3, %7, %11, %16, 85; bra.uni GLE;\n"
-        "GL86: lop3.b32 %0, %4, %8, %13, 86; lop3.b32 %1, %5, %9, %14, 86; lop3.b32 %2, %6, %10, %15, 86; lop3.b32 %3, %7, %11, %16, 86; bra.uni GLE;\n"
-        "GL87: lop3.b32 %0, %4, %8, %13, 87; lop3.b32 %1, %5, %9, %14, 87; lop3.b32 %2, %6, %10, %15, 87; lop3.b32 %3, %7, %11, %16, 87; bra.uni GLE;\n"
-        "GL88: lop3.b32 %0, %4, %8, %13, 88; lop3.b32 %1, %5, %9, %14, 88; lop3.b32 %2, %6, %10, %15, 88; lop3.b32 %3, %7, %11, %16, 88; bra.uni GLE;\n"
-        "GL89: lop3.b32 %0, %4, %8, %13, 89; lop3.b32 %1, %5, %9, %14, 89; lop3.b32 %2, %6, %10, %15, 89; lop3.b32 %3, %7, %11, %16, 89; bra.uni GLE;\n"
-        "GL90: lop3.b32 %0, %4, %8, %13, 90; lop3.b32 %1, %5, %9, %14, 90; lop3.b32 %2, %6, %10, %15, 90; lop3.b32 %3, %7, %11, %16, 90; bra.uni GLE;\n"
-        "GL91: lop3.b32 %0, %4, %8, %13, 91; lop3.b32 %1, %5, %9, %14, 91; lop3.b32 %2, %6, %10, %15, 91; lop3.b32 %3, %7, %11, %16, 91; bra.uni GLE;\n"
-        "GL92: lop3.b32 %0, %4, %8, %13, 92; lop3.b32 %1, %5, %9, %14, 92; lop3.b32 %2, %6, %10, %15, 92; lop3.b32 %3, %7, %11, %16, 92; bra.uni GLE;\n"
-        "GL93: lop3.b32 %0, %4, %8, %13, 93; lop3.b32 %1, %5, %9, %14, 93; lop3.b32 %2, %6, %10, %15, 93; lop3.b32 %3, %7, %11, %16, 93; bra.uni GLE;\n"
-        "GL94: lop3.b32 %0, %4, %8, %13, 94; lop3.b32 %1, %5, %9, %14, 94; lop3.b32 %2, %6, %10, %15, 94; lop3.b32 %3, %7, %11, %16, 94; bra.uni GLE;\n"
-        "GL95: lop3.b32 %0, %4, %8, %13, 95; lop3.b32 %1, %5, %9, %14, 95; lop3.b32 %2, %6, %10, %15, 95; lop3.b32 %3, %7, %11, %16, 95; bra.uni GLE;\n"
-        "GL96: lop3.b32 %0, %4, %8, %13, 96; lop3.b32 %1, %5, %9, %14, 96; lop3.b32 %2, %6, %10, %15, 96; lop3.b32 %3, %7, %11, %16, 96; bra.uni GLE;\n"
-        "GL97: lop3.b32 %0, %4, %8, %13, 97; lop3.b32 %1, %5, %9, %14, 97; lop3.b32 %2, %6, %10, %15, 97; lop3.b32 %3, %7, %11, %16, 97; bra.uni GLE;\n"
-        "GL98: lop3.b32 %0, %4, %8, %13, 98; lop3.b32 %1, %5, %9, %14, 98; lop3.b32 %2, %6, %10, %15, 98; lop3.b32 %3, %7, %11, %16, 98; bra.uni GLE;\n"
-        "GL99: lop3.b32 %0, %4, %8, %13, 99; lop3.b32 %1, %5, %9, %14, 99; lop3.b32 %2, %6, %10, %15, 99; lop3.b32 %3, %7, %11, %16, 99; bra.uni GLE;\n"
-        "GL100: lop3.b32 %0, %4, %8, %13, 100; lop3.b32 %1, %5, %9, %14, 100; lop3.b32 %2, %6, %10, %15, 100; lop3.b32 %3, %7, %11, %16, 100; bra.uni GLE;\n"
-        "GL101: lop3.b32 %0, %4, %8, %13, 101; lop3.b32 %1, %5, %9, %14, 101; lop3.b32 %2, %6, %10, %15, 101; lop3.b32 %3, %7, %11, %16, 101; bra.uni GLE;\n"
-        "GL102: lop3.b32 %0, %4, %8, %13, 102; lop3.b32 %1, %5, %9, %14, 102; lop3.b32 %2, %6, %10, %15, 102; lop3.b32 %3, %7, %11, %16, 102; bra.uni GLE;\n"
-        "GL103: lop3.b32 %0, %4, %8, %13, 103; lop3.b32 %1, %5, %9, %14, 103; lop3.b32 %2, %6, %10, %15, 103; lop3.b32 %3, %7, %11, %16, 103; bra.uni GLE;\n"
-        "GL104: lop3.b32 %0, %4, %8, %13, 104; lop3.b32 %1, %5, %9, %14, 104; lop3.b32 %2, %6, %10, %15, 104; lop3.b32 %3, %7, %11, %16, 104; bra.uni GLE;\n"
-        "GL105: lop3.b32 %0, %4, %8, %13, 105; lop3.b32 %1, %5, %9, %14, 105; lop3.b32 %2, %6, %10, %15, 105; lop3.b32 %3, %7, %11, %16, 105; bra.uni GLE;\n"
-        "GL106: lop3.b32 %0, %4, %8, %13, 106; lop3.b32 %1, %5, %9, %14, 106; lop3.b32 %2, %6, %10, %15, 106; lop3.b32 %3, %7, %11, %16, 106; bra.uni GLE;\n"
-        "GL107: lop3.b32 %0, %4, %8, %13, 107; lop3.b32 %1, %5, %9, %14, 107; lop3.b32 %2, %6, %10, %15, 107; lop3.b32 %3, %7, %11, %16, 107; bra.uni GLE;\n"
-        "GL108: lop3.b32 %0, %4, %8, %13, 108; lop3.b32 %1, %5, %9, %14, 108; lop3.b32 %2, %6, %10, %15, 108; lop3.b32 %3, %7, %11, %16, 108; bra.uni GLE;\n"
-        "GL109: lop3.b32 %0, %4, %8, %13, 109; lop3.b32 %1, %5, %9, %14, 109; lop3.b32 %2, %6, %10, %15, 109; lop3.b32 %3, %7, %11, %16, 109; bra.uni GLE;\n"
-        "GL110: lop3.b32 %0, %4, %8, %13, 110; lop3.b32 %1, %5, %9, %14, 110; lop3.b32 %2, %6, %10, %15, 110; lop3.b32 %3, %7, %11, %16, 110; bra.uni GLE;\n"
-        "GL111: lop3.b32 %0, %4, %8, %13, 111; lop3.b32 %1, %5, %9, %14, 111; lop3.b32 %2, %6, %10, %15, 111; lop3.b32 %3, %7, %11, %16, 111; bra.uni GLE;\n"
-        "GL112: lop3.b32 %0, %4, %8, %13, 112; lop3.b32 %1, %5, %9, %14, 112; lop3.b32 %2, %6, %10, %15, 112; lop3.b32 %3, %7, %11, %16, 112; bra.uni GLE;\n"
-        "GL113: lop3.b32 %0, %4, %8, %13, 113; lop3.b32 %1, %5, %9, %14, 113; lop3.b32 %2, %6, %10, %15, 113; lop3.b32 %3, %7, %11, %16, 113; bra.uni GLE;\n"
-        "GL114: lop3.b32 %0, %4, %8, %13, 114; lop3.b32 %1, %5, %9, %14, 114; lop3.b32 %2, %6, %10, %15, 114; lop3.b32 %3, %7, %11, %16, 114; bra.uni GLE;\n"
-        "GL115: lop3.b32 %0, %4, %8, %13, 115; lop3.b32 %1, %5, %9, %14, 115; lop3.b32 %2, %6, %10, %15, 115; lop3.b32 %3, %7, %11, %16, 115; bra.uni GLE;\n"
-        "GL116: lop3.b32 %0, %4, %8, %13, 116; lop3.b32 %1, %5, %9, %14, 116; lop3.b32 %2, %6, %10, %15, 116; lop3.b32 %3, %7, %11, %16, 116; bra.uni GLE;\n"
-        "GL117: lop3.b32 %0, %4, %8, %13, 117; lop3.b32 %1, %5, %9, %14, 117; lop3.b32 %2, %6, %10, %15, 117; lop3.b32 %3, %7, %11, %16, 117; bra.uni GLE;\n"
-        "GL118: lop3.b32 %0, %4, %8, %13, 118; lop3.b32 %1, %5, %9, %14, 118; lop3.b32 %2, %6, %10, %15, 118; lop3.b32 %3, %7, %11, %16, 118; bra.uni GLE;\n"
-        "GL119: lop3.b32 %0, %4, %8, %13, 119; lop3.b32 %1, %5, %9, %14, 119; lop3.b32 %2, %6, %10, %15, 119; lop3.b32 %3, %7, %11, %16, 119; bra.uni GLE;\n"
-        "GL120: lop3.b32 %0, %4, %8, %13, 120; lop3.b32 %1, %5, %9, %14, 120; lop3.b32 %2, %6, %10, %15, 120; lop3.b32 %3, %7, %11, %16, 120; bra.uni GLE;\n"
-        "GL121: lop3.b32 %0, %4, %8, %13, 121; lop3.b32 %1, %5, %9, %14, 121; lop3.b32 %2, %6, %10, %15, 121; lop3.b32 %3, %7, %11, %16, 121; bra.uni GLE;\n"
-        "GL122: lop3.b32 %0, %4, %8, %13, 122; lop3.b32 %1, %5, %9, %14, 122; lop3.b32 %2, %6, %10, %15, 122; lop3.b32 %3, %7, %11, %16, 122; bra.uni GLE;\n"
-        "GL123: lop3.b32 %0, %4, %8, %13, 123; lop3.b32 %1, %5, %9, %14, 123; lop3.b32 %2, %6, %10, %15, 123; lop3.b32 %3, %7, %11, %16, 123; bra.uni GLE;\n"
-        "GL124: lop3.b32 %0, %4, %8, %13, 124; lop3.b32 %1, %5, %9, %14, 124; lop3.b32 %2, %6, %10, %15, 124; lop3.b32 %3, %7, %11, %16, 124; bra.uni GLE;\n"
-        "GL125: lop3.b32 %0, %4, %8, %13, 125; lop3.b32 %1, %5, %9, %14, 125; lop3.b32 %2, %6, %10, %15, 125; lop3.b32 %3, %7, %11, %16, 125; bra.uni GLE;\n"
-        "GL126: lop3.b32 %0, %4, %8, %13, 126; lop3.b32 %1, %5, %9, %14, 126; lop3.b32 %2, %6, %10, %15, 126; lop3.b32 %3, %7, %11, %16, 126; bra.uni GLE;\n"
-        "GL127: lop3.b32 %0, %4, %8, %13, 127; lop3.b32 %1, %5, %9, %14, 127; lop3.b32 %2, %6, %10, %15, 127; lop3.b32 %3, %7, %11, %16, 127; bra.uni GLE;\n"
+        ISING_GL_ALL(ISING_GL_CASE)
         "GLE:\n"
         "}\n"
         : "=r"(T.x), "=r"(T.y), "=r"(T.z), "=r"(T.w)
@@ -319,6 +205,11 @@ __device__ __forceinline__ uint4 class_select(const uint32_t lut, const uint4 c2
           "r"(c0.x), "r"(c0.y), "r"(c0.z), "r"(c0.w));
     return T;
 }
+#undef ISING_GL_ALL
+#undef ISING_GL_ROW
+#undef ISING_GL_CASE
+#undef ISING_GL_TGT
+#undef ISING_GL_LBL
 
 // 32 x 32 -> 64 bit product as ONE IMAD.WIDE.U32 (written in PTX: inside the plane loop the C++
 // form picked up a dead add per product)
